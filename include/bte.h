@@ -1,0 +1,123 @@
+/* include/bte.h -- C-ABI boundary of the B200-native phonon-BTE sweep library.
+ *
+ * What it computes (arxiv 2503.23657 "JAX-BTE", /root/reference/PAPER.md):
+ * the forward solver's hot path -- nongray RTA phonon BTE in energy-deviation form
+ * (Eq. 15) advanced by source iteration (steps 1-4):
+ * every iteration runs an upwind finite-volume discrete-ordinates sweep for every
+ * (band, direction) (exact solve of Eq. 20 with the first-order A of Eq. 21,
+ * PAPER.md:270-279, on a Cartesian / voxel-masked grid), accumulates the 0th/1st
+ * angular moments inside the sweep, then updates the lattice temperature (Eq. 16,
+ * PAPER.md:244-247), the heat flux (Eq. 4) and the residuals (Eq. 23,
+ * PAPER.md:299-304).  Boundary inflow follows Eq. 5-7 plus a
+ * periodic wrap, always taken from the previous iteration (lagged store).
+ *
+ * Conventions
+ *  - all functions are extern "C", return a bte_status, never throw, never abort;
+ *  - arrays are x fastest: idx = i + nx*(j + ny*k);
+ *  - "host" / "device" in a comment says where a pointer must live;
+ *  - OWNERSHIP: the caller owns the device workspace and every output buffer and keeps
+ *    them alive until bte_destroy; host input arrays are copied during bte_create and may
+ *    be freed afterwards; the library calls no cudaMalloc after bte_create returns and none
+ *    on the hot path (it allocates nothing on the device at all: everything lives in the
+ *    caller's workspace);
+ *  - cuda_stream is a cudaStream_t passed as void* (NULL = legacy default stream);
+ *  - a handle is not thread-safe; different handles are independent, but handles that
+ *    iterate concurrently on different streams of one device are NOT supported (they share
+ *    one __constant__ coefficient bank, re-uploaded in stream order by bte_iterate);
+ *  - there is no CPU fallback: without a CUDA device every compute entry point returns
+ *    BTE_ERR_CUDA.
+ */
+#ifndef BTE_H
+#define BTE_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bte_solver bte_solver; /* opaque */
+
+typedef enum {
+  BTE_OK = 0,
+  BTE_ERR_INVALID_ARG = 1, /* sizes <= 0, C/v/tau <= 0, non-unit s, unpaired PERIODIC, dim/nz mismatch,
+                              no solid cell, interface_bc PERIODIC, NULL where a pointer is required */
+  BTE_ERR_QUADRATURE = 2,  /* |sum w - 4pi| > 1e-6*4pi; a SPECULAR face whose axis reflection does not
+                              map the direction set onto itself (with equal weights) */
+  BTE_ERR_WORKSPACE = 3,   /* workspace NULL, misaligned (256 B) or smaller than bte_workspace_bytes */
+  BTE_ERR_CUDA = 4,        /* any CUDA runtime error (bte_last_cuda_error gives the code) */
+  BTE_ERR_UNSUPPORTED = 5  /* valid problem outside this build: SPECULAR interface_bc; coefficient table
+                              larger than the constant bank (non-mirror-symmetric quadrature x many bands) */
+} bte_status;
+
+/* Eq. 5 / Eq. 6 / Eq. 7; PERIODIC: BASELINE.json configs[3] */
+typedef enum { BTE_BC_ISOTHERMAL = 0, BTE_BC_DIFFUSE = 1, BTE_BC_SPECULAR = 2, BTE_BC_PERIODIC = 3 } bte_bc_type;
+
+/* BTE_FP64: everything fp64.  BTE_FP32_STORE_FP64_ACC: cell inputs, tables, recurrence, wavefront
+ * buffers and the lagged boundary store in fp32; the moment sum over the <=16 directions of one
+ * (octant, band) work item is an fp32 partial, every further sum (bands, octants, cells, residual
+ * norms) and the dT division are fp64 (reading G15). */
+typedef enum { BTE_FP64 = 0, BTE_FP32_STORE_FP64_ACC = 1 } bte_precision;
+
+typedef struct { int32_t type; double dT_wall; } bte_bc; /* dT_wall [K] used by ISOTHERMAL only */
+
+typedef struct {
+  int32_t nx, ny, nz, dim;   /* dim=1: x only (ny=nz=1); 2: x,y (nz=1); 3: x,y,z */
+  double dx, dy, dz;         /* metres; only the first `dim` are used */
+  const uint8_t *solid_mask; /* host, nx*ny*nz, 1 = solid; NULL = all solid */
+  int32_t n_bands;
+  const double *C, *v, *tau; /* host, [n_bands]; J/m^3K, m/s, s; all > 0 */
+  int32_t n_dirs;
+  const double *s;           /* host, [n_dirs][3] unit vectors */
+  const double *w;           /* host, [n_dirs], sum = 4 pi */
+  bte_bc face_bc[6];         /* x-, x+, y-, y+, z-, z+ ; PERIODIC must be set on both faces of an axis */
+  bte_bc interface_bc;       /* every solid/void face inside the box (ISOTHERMAL or DIFFUSE) */
+  const double *Q;           /* host, nx*ny*nz, W/m^3; NULL = 0 */
+  int32_t precision;         /* bte_precision */
+} bte_problem;
+
+/* Bytes of device workspace bte_create needs for this problem; 0 if the problem is invalid. */
+size_t bte_workspace_bytes(const bte_problem *p);
+
+/* Validate, build the sweep schedule, upload tables into d_workspace (device, 256-B aligned,
+ * >= bte_workspace_bytes), initialise dT = 0 and the lagged store = 0.  Synchronises the stream
+ * before returning.  *out is untouched on failure. */
+bte_status bte_create(const bte_problem *p, void *d_workspace, size_t bytes, void *cuda_stream, bte_solver **out);
+
+/* n source iterations (sweep of all (band,direction) + moments + dT/q/residual update), asynchronous
+ * on cuda_stream; n >= 0. */
+bte_status bte_iterate(bte_solver *h, int32_t n, void *cuda_stream);
+
+/* dT [K] (deviation from the reference temperature) per cell, fp64 in both precisions, void cells 0.
+ * d_out: device, [nx*ny*nz]. Asynchronous on cuda_stream. */
+bte_status bte_get_temperature(bte_solver *h, double *d_out, void *cuda_stream);
+/* q [W/m^2], cell-centred (Eq. 4). d_out: device, [3][nx*ny*nz]. Asynchronous. */
+bte_status bte_get_heat_flux(bte_solver *h, double *d_out, void *cuda_stream);
+/* Overwrite dT (restart / tests). d_in: device, [nx*ny*nz]. Asynchronous. */
+bte_status bte_set_temperature(bte_solver *h, const double *d_in, void *cuda_stream);
+
+/* eps_T, eps_q of the last iteration (Eq. 23; normalised by max|dT|, max|q| over
+ * solid cells; 0/0 -> 0, x/0 -> +inf; +inf before the first iteration). Host outputs (may be NULL).
+ * SYNCHRONISES the stream last used by bte_iterate. */
+bte_status bte_residual(bte_solver *h, double *eps_T, double *eps_q);
+
+/* Whole-path convenience with HOST buffers (used for end-to-end timing): uploads Q (host, [nx*ny*nz],
+ * may be NULL = keep), resets dT and the store to 0, runs n iterations, downloads dT (host [nx*ny*nz])
+ * and q (host [3][nx*ny*nz]; may be NULL). Synchronous. */
+bte_status bte_solve_host(bte_solver *h, const double *Q_host, int32_t n, double *dT_host, double *q_host,
+                          void *cuda_stream);
+
+int64_t bte_updates_per_sweep(const bte_solver *h); /* solid cells * n_bands * n_dirs */
+int64_t bte_iterations_done(const bte_solver *h);
+int32_t bte_kernel_launches_per_iteration(const bte_solver *h);
+/* schedule facts for reporting: out[0]=work units per sweep, [1]=CTAs launched, [2]=threads per CTA,
+ * [3]=wavefront steps summed over units, [4]=thread-slot updates issued per sweep (occupancy
+ * denominator: useful updates / this), [5]=bytes of workspace in use */
+void bte_schedule_info(const bte_solver *h, int64_t out[6]);
+void bte_destroy(bte_solver *h);
+const char *bte_status_string(bte_status s);
+int32_t bte_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
