@@ -1,0 +1,534 @@
+// Host side of the B200 phonon-BTE sweep library: validation, sweep schedule, workspace
+// carve-up and the extern "C" entry points declared in include/bte.h.
+// Product code: shares nothing with oracle/.  No CPU fallback: every compute entry point
+// needs a CUDA device.
+#include "../../include/bte.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <limits>
+#include <map>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "bte_kernels.cuh"
+
+static thread_local int g_last_cuda = 0;
+#define CK(call)                                                       \
+  do {                                                                 \
+    cudaError_t e_ = (call);                                           \
+    if (e_ != cudaSuccess) { g_last_cuda = (int)e_; return BTE_ERR_CUDA; } \
+  } while (0)
+
+namespace {
+
+const double kFourPi = 12.566370614359172953850573533118;
+
+struct Plan {
+  BteDev dev{};                          // geometry part filled by build_plan, pointers by carve()
+  std::vector<uint8_t> code;             // [ncell]
+  std::vector<int32_t> iface, iface_info;
+  std::vector<double> Q;                 // [ncell]
+  std::vector<double> band;              // [4][B]
+  std::vector<double> coef;              // unique coefficient blocks, 16x8 doubles each
+  std::vector<int32_t> item_coef;        // [8][max_items]
+  std::vector<BteUnit> units;
+  double sumC = 0;
+  int nthreads = 32;
+  size_t smem = 0;
+  int64_t steps_total = 0;
+  // workspace offsets
+  size_t total = 0, state_begin = 0, state_end = 0;
+  bool any_diffuse_face = false;
+  size_t gf_elems = 0;
+  size_t xpl_elems[8]{}, ypl_elems[8]{}, zpl_elems[8]{};
+};
+
+size_t align_up(size_t x) { return (x + 255) & ~size_t(255); }
+
+bte_status build_plan(const bte_problem *p, Plan &pl) {
+  if (!p) return BTE_ERR_INVALID_ARG;
+  if (p->nx < 1 || p->ny < 1 || p->nz < 1 || p->dim < 1 || p->dim > 3) return BTE_ERR_INVALID_ARG;
+  if ((p->dim < 3 && p->nz != 1) || (p->dim < 2 && p->ny != 1)) return BTE_ERR_INVALID_ARG;
+  if (p->n_bands < 1 || p->n_dirs < 1 || !p->C || !p->v || !p->tau || !p->s || !p->w) return BTE_ERR_INVALID_ARG;
+  if (p->precision != BTE_FP64 && p->precision != BTE_FP32_STORE_FP64_ACC) return BTE_ERR_INVALID_ARG;
+  const double delta[3] = {p->dx, p->dy, p->dz};
+  for (int a = 0; a < p->dim; ++a)
+    if (!(delta[a] > 0.0) || !std::isfinite(delta[a])) return BTE_ERR_INVALID_ARG;
+  const int B = p->n_bands, D = p->n_dirs;
+  for (int b = 0; b < B; ++b)
+    if (!(p->C[b] > 0) || !(p->v[b] > 0) || !(p->tau[b] > 0)) return BTE_ERR_INVALID_ARG;
+  double sw = 0;
+  for (int d = 0; d < D; ++d) {
+    const double *s = p->s + 3 * d;
+    if (std::fabs(s[0] * s[0] + s[1] * s[1] + s[2] * s[2] - 1.0) > 1e-9) return BTE_ERR_INVALID_ARG;
+    if (!(p->w[d] >= 0)) return BTE_ERR_INVALID_ARG;
+    sw += p->w[d];
+  }
+  if (std::fabs(sw - kFourPi) > 1e-6 * kFourPi) return BTE_ERR_QUADRATURE;
+  for (int a = 0; a < p->dim; ++a) {
+    const int t0 = p->face_bc[2 * a].type, t1 = p->face_bc[2 * a + 1].type;
+    if (t0 < 0 || t0 > 3 || t1 < 0 || t1 > 3) return BTE_ERR_INVALID_ARG;
+    if ((t0 == BTE_BC_PERIODIC) != (t1 == BTE_BC_PERIODIC)) return BTE_ERR_INVALID_ARG;
+  }
+  if (p->interface_bc.type == BTE_BC_PERIODIC || p->interface_bc.type < 0 || p->interface_bc.type > 3)
+    return BTE_ERR_INVALID_ARG;
+
+  BteDev &dv = pl.dev;
+  dv.nx = p->nx; dv.ny = p->ny; dv.nz = p->nz; dv.dim = p->dim;
+  dv.B = B; dv.n_dirs = D;
+  dv.fp32 = p->precision == BTE_FP32_STORE_FP64_ACC;
+  dv.has_y = p->dim >= 2; dv.has_z = p->dim >= 3;
+  dv.TZ = dv.has_z ? (p->nz > 8 ? 16 : 8) : 1;
+  dv.nty = (p->ny + 31) / 32; dv.ntz = (p->nz + dv.TZ - 1) / dv.TZ;
+  dv.NU = p->nx + 31; dv.nyp = dv.nty * 32;
+  dv.ncell = (int64_t)p->nx * p->ny * p->nz;
+  dv.NS = (int64_t)p->nz * dv.nty * dv.NU * 32;
+  pl.nthreads = 32 * dv.TZ;
+  const size_t tsz = dv.fp32 ? 4 : 8;
+  pl.smem = (size_t)(2 * (dv.TZ + 1) * BTE_P * 32 + 2 * dv.TZ * BTE_P) * tsz;
+
+  // ---- cells: solid mask, interface bits, interface faces
+  const int64_t N = dv.ncell;
+  const int n[3] = {p->nx, p->ny, p->nz};
+  pl.code.assign((size_t)N, 0);
+  int64_t nsolid = 0;
+  for (int64_t c = 0; c < N; ++c) {
+    const bool s = p->solid_mask ? p->solid_mask[c] != 0 : true;
+    pl.code[c] = s ? BTE_CODE_SOLID : 0;
+    nsolid += s;
+  }
+  if (nsolid == 0) return BTE_ERR_INVALID_ARG;
+  dv.nsolid = nsolid;
+  std::vector<int32_t> iface;
+  if (p->solid_mask) iface.assign((size_t)6 * N, -1);
+  int32_t nif = 0;
+  if (p->solid_mask) {
+    for (int k = 0; k < n[2]; ++k) for (int j = 0; j < n[1]; ++j) for (int i = 0; i < n[0]; ++i) {
+      const int64_t c = i + (int64_t)n[0] * (j + (int64_t)n[1] * k);
+      if (!(pl.code[c] & BTE_CODE_SOLID)) continue;
+      const int ijk[3] = {i, j, k};
+      for (int f = 0; f < 2 * p->dim; ++f) {
+        const int a = f >> 1;
+        int u[3] = {i, j, k};
+        u[a] = ijk[a] + ((f & 1) ? 1 : -1);
+        if (u[a] < 0 || u[a] >= n[a]) {
+          if (p->face_bc[f].type != BTE_BC_PERIODIC) continue;   // box face: handled by ghost planes
+          u[a] = (u[a] + n[a]) % n[a];
+        }
+        const int64_t uc = u[0] + (int64_t)n[0] * (u[1] + (int64_t)n[1] * u[2]);
+        if (pl.code[uc] & BTE_CODE_SOLID) continue;
+        pl.code[c] |= (uint8_t)(2 << f);
+        iface[(size_t)f * N + c] = nif++;
+        pl.iface_info.push_back(f);
+      }
+    }
+  }
+  dv.n_iface = nif;
+  if (nif > 0) {
+    if (p->interface_bc.type == BTE_BC_SPECULAR) return BTE_ERR_UNSUPPORTED;
+    pl.iface.swap(iface);
+  }
+  dv.iface_type = p->interface_bc.type; dv.iface_dT = p->interface_bc.dT_wall;
+  for (int f = 0; f < 6; ++f) {
+    dv.face_type[f] = p->face_bc[f].type; dv.face_dT[f] = p->face_bc[f].dT_wall;
+    const int a = f >> 1;
+    const double ns = (f & 1) ? 1.0 : -1.0;
+    double Pi = 0;
+    for (int d = 0; d < D; ++d) { const double sn = ns * p->s[3 * d + a]; if (sn < 0) Pi -= p->w[d] * sn; }
+    dv.Pi_face[f] = Pi;
+    if (f < 2 * p->dim && p->face_bc[f].type == BTE_BC_DIFFUSE) pl.any_diffuse_face = true;
+  }
+  pl.Q.assign((size_t)N, 0.0);
+  if (p->Q) for (int64_t c = 0; c < N; ++c) pl.Q[c] = p->Q[c];
+
+  // ---- bands
+  double sumC = 0, sumCt = 0;
+  for (int b = 0; b < B; ++b) { sumC += p->C[b]; sumCt += p->C[b] / p->tau[b]; }
+  pl.sumC = sumC;
+  dv.inv_sumCtau = 1.0 / sumCt;
+  pl.band.assign((size_t)4 * B, 0.0);
+  for (int b = 0; b < B; ++b) {
+    pl.band[b] = p->C[b] / kFourPi;                              // e0 = C dT / 4pi (Eq. 16)
+    pl.band[B + b] = p->C[b] * p->tau[b] / kFourPi;              // x (Q / sumC): tau Q_b / 4pi (Eq. 11, 15)
+    pl.band[2 * B + b] = 1.0 / p->tau[b];
+    pl.band[3 * B + b] = p->v[b];
+  }
+
+  // ---- directions -> octants, canonical order inside an octant (by |s|), 16-slot chunks
+  std::vector<int> od[8];
+  for (int d = 0; d < D; ++d) {
+    const double *s = p->s + 3 * d;
+    od[(s[0] < 0) | ((s[1] < 0) << 1) | ((s[2] < 0) << 2)].push_back(d);
+  }
+  auto key = [&](int d, int a) { return std::llround(std::fabs(p->s[3 * d + a]) * 1e11); };
+  for (int o = 0; o < 8; ++o)
+    std::sort(od[o].begin(), od[o].end(), [&](int x, int y) {
+      for (int a = 0; a < 3; ++a) if (key(x, a) != key(y, a)) return key(x, a) < key(y, a);
+      return x < y;
+    });
+  for (int a = 0; a < p->dim; ++a) {
+    if (p->face_bc[2 * a].type != BTE_BC_SPECULAR && p->face_bc[2 * a + 1].type != BTE_BC_SPECULAR) continue;
+    for (int o = 0; o < 8; ++o) {
+      const std::vector<int> &A = od[o], &M = od[o ^ (1 << a)];
+      if (A.size() != M.size()) return BTE_ERR_QUADRATURE;
+      for (size_t q = 0; q < A.size(); ++q) {
+        for (int c = 0; c < 3; ++c)
+          if (std::fabs(std::fabs(p->s[3 * A[q] + c]) - std::fabs(p->s[3 * M[q] + c])) > 1e-12) return BTE_ERR_QUADRATURE;
+        if (std::fabs(p->w[A[q]] - p->w[M[q]]) > 1e-12 * kFourPi) return BTE_ERR_QUADRATURE;
+      }
+    }
+  }
+  int max_items = 1, max_chunk = 1;
+  for (int o = 0; o < 8; ++o) {
+    BteOct &O = dv.oct[o];
+    O.sx = (o & 1) ? -1 : 1; O.sy = (o & 2) ? -1 : 1; O.sz = (o & 4) ? -1 : 1;
+    O.cls = o & 3;
+    O.active = !od[o].empty();
+    O.nchunk = ((int)od[o].size() + BTE_P - 1) / BTE_P;
+    O.nitems = O.nchunk * B;
+    max_items = std::max(max_items, O.nitems);
+    max_chunk = std::max(max_chunk, O.nchunk);
+  }
+  dv.max_items = max_items;
+  dv.nHslot = 4 * max_chunk;
+  pl.item_coef.assign((size_t)8 * max_items, 0);
+  std::map<std::string, int32_t> seen;
+  for (int o = 0; o < 8; ++o) {
+    const BteOct &O = dv.oct[o];
+    for (int b = 0; b < B; ++b) for (int c = 0; c < O.nchunk; ++c) {
+      double blk[BTE_P * BTE_NCOEF];
+      std::memset(blk, 0, sizeof blk);
+      const double Lam = p->v[b] * p->tau[b];
+      for (int q = 0; q < BTE_P; ++q) {
+        const size_t pos = (size_t)c * BTE_P + q;
+        if (pos >= od[o].size()) break;
+        const int d = od[o][pos];
+        double ca[3] = {0, 0, 0}, sum = 1.0;
+        for (int a = 0; a < p->dim; ++a) { ca[a] = Lam * std::fabs(p->s[3 * d + a]) / delta[a]; sum += ca[a]; }
+        const double inv = 1.0 / sum;     // row i of Eq. 21 scaled by tau: (1 + sum_a c_a) e = rhs + sum_a c_a e_up
+        double *r = blk + q * BTE_NCOEF;
+        r[0] = inv; r[1] = ca[0] * inv; r[2] = ca[1] * inv; r[3] = ca[2] * inv;
+        r[4] = p->w[d];
+        for (int a = 0; a < 3; ++a) r[5 + a] = p->w[d] * std::fabs(p->s[3 * d + a]);
+      }
+      const std::string k((const char *)blk, sizeof blk);
+      auto it = seen.find(k);
+      int32_t off;
+      if (it == seen.end()) {
+        off = (int32_t)pl.coef.size();
+        pl.coef.insert(pl.coef.end(), blk, blk + BTE_P * BTE_NCOEF);
+        seen.emplace(k, off);
+      } else off = it->second;
+      pl.item_coef[(size_t)o * max_items + b * O.nchunk + c] = off;
+    }
+  }
+  if (pl.coef.size() * tsz > BTE_CONST_BYTES) return BTE_ERR_UNSUPPORTED;
+
+  // ---- work units in ticket (topological) order: key = item + ty + tz
+  struct Key { int key, o, item, ty, tz; };
+  std::vector<Key> ks;
+  for (int o = 0; o < 8; ++o) {
+    if (!dv.oct[o].active) continue;
+    for (int it = 0; it < dv.oct[o].nitems; ++it)
+      for (int ty = 0; ty < dv.nty; ++ty) for (int tz = 0; tz < dv.ntz; ++tz) ks.push_back({it + ty + tz, o, it, ty, tz});
+  }
+  std::stable_sort(ks.begin(), ks.end(), [](const Key &a, const Key &b) { return a.key < b.key; });
+  std::vector<int32_t> idmap((size_t)8 * max_items * dv.nty * dv.ntz, -1);
+  auto slot = [&](int o, int it, int ty, int tz) { return (((size_t)o * max_items + it) * dv.nty + ty) * dv.ntz + tz; };
+  for (size_t u = 0; u < ks.size(); ++u) idmap[slot(ks[u].o, ks[u].item, ks[u].ty, ks[u].tz)] = (int32_t)u;
+  pl.units.resize(ks.size());
+  for (size_t u = 0; u < ks.size(); ++u) {
+    const Key &k = ks[u];
+    BteUnit &U = pl.units[u];
+    U.oct = k.o; U.item = k.item; U.ty = k.ty; U.tz = k.tz;
+    U.band = k.item / dv.oct[k.o].nchunk; U.chunk = k.item % dv.oct[k.o].nchunk;
+    U.coef_off = pl.item_coef[(size_t)k.o * max_items + k.item];
+    U.dep_y = k.ty > 0 ? idmap[slot(k.o, k.item, k.ty - 1, k.tz)] : -1;
+    U.dep_z = k.tz > 0 ? idmap[slot(k.o, k.item, k.ty, k.tz - 1)] : -1;
+    U.dep_prev = k.item > 0 ? idmap[slot(k.o, k.item - 1, k.ty, k.tz)] : -1;
+  }
+  dv.n_units = (int32_t)pl.units.size();
+  pl.steps_total = (int64_t)pl.units.size() * (dv.nx + 31 + dv.TZ - 1);
+
+  // ---- workspace carve-up (offsets only; pointers are set in bind())
+  pl.gf_elems = 0;
+  for (int f = 0; f < 2 * p->dim; ++f) {
+    const int a = f >> 1;
+    const int64_t na = a == 0 ? p->ny : p->nx, nb = a == 2 ? p->ny : p->nz;
+    pl.gf_elems += (size_t)na * nb * B;
+  }
+  for (int o = 0; o < 8; ++o) {
+    const BteOct &O = dv.oct[o];
+    if (!O.active) continue;
+    pl.xpl_elems[o] = (size_t)2 * O.nitems * BTE_P * dv.nz * dv.nyp;
+    pl.ypl_elems[o] = dv.has_y ? (size_t)(dv.nty + 1) * O.nitems * dv.nz * dv.nx * BTE_P : 0;
+    pl.zpl_elems[o] = dv.has_z ? (size_t)(dv.ntz + 1) * O.nitems * dv.nty * dv.NU * BTE_P * 32 : 0;
+  }
+  dv.n_red_blocks = (int)std::min<int64_t>((N + 255) / 256, 148 * 8);
+  return BTE_OK;
+}
+
+// Assign device pointers inside the workspace. Returns total bytes needed.
+size_t bind(Plan &pl, unsigned char *ws) {
+  BteDev &dv = pl.dev;
+  const size_t tsz = dv.fp32 ? 4 : 8;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { void *p = ws ? ws + off : nullptr; off = align_up(off + bytes); return p; };
+  const size_t N = (size_t)dv.ncell, NS = (size_t)dv.NS;
+  dv.code = (uint8_t *)take(N);
+  for (int c = 0; c < 4; ++c) dv.code_sk[c] = (uint8_t *)take(NS);
+  for (int c = 0; c < 4; ++c) dv.Q_sk[c] = take(NS * tsz);
+  dv.Qphys = (double *)take(N * 8);
+  dv.iface = dv.n_iface ? (int32_t *)take((size_t)6 * N * 4) : nullptr;
+  dv.iface_info = dv.n_iface ? (int32_t *)take((size_t)dv.n_iface * 4) : nullptr;
+  dv.item_coef = (const int32_t *)take((size_t)8 * dv.max_items * 4);
+  dv.units = (BteUnit *)take((size_t)dv.n_units * sizeof(BteUnit));
+  dv.band = (double *)take((size_t)4 * dv.B * 8);
+  // ---- state (reset to 0 by bte_solve_host)
+  pl.state_begin = off;
+  dv.done = (int32_t *)take((size_t)dv.n_units * 4);
+  dv.ticket = (int32_t *)take(256);
+  dv.red = (double *)take((size_t)(4 * dv.n_red_blocks + 4) * 8);
+  for (int c = 0; c < 4; ++c) dv.dT_sk[c] = take(NS * tsz);
+  dv.dT = (double *)take(N * 8);
+  dv.q = (double *)take(3 * N * 8);
+  dv.qmag = (double *)take(N * 8);
+  dv.Gi = dv.n_iface ? take((size_t)dv.n_iface * dv.B * tsz) : nullptr;
+  dv.Hpart = dv.n_iface ? (double *)take((size_t)dv.n_iface * dv.B * dv.nHslot * 8) : nullptr;
+  dv.Gf = take(std::max<size_t>(pl.gf_elems, 1) * tsz);
+  for (int o = 0; o < 8; ++o) {
+    BteOct &O = dv.oct[o];
+    if (!O.active) { O.M = nullptr; O.xpl = O.ypl = O.zpl = nullptr; continue; }
+    O.M = (double *)take(4 * NS * 8);
+    O.xpl = take(pl.xpl_elems[o] * tsz);
+    O.ypl = pl.ypl_elems[o] ? take(pl.ypl_elems[o] * tsz) : nullptr;
+    O.zpl = pl.zpl_elems[o] ? take(pl.zpl_elems[o] * tsz) : nullptr;
+  }
+  pl.state_end = off;
+  pl.total = off;
+  return off;
+}
+
+}  // namespace
+
+struct bte_solver {
+  Plan pl;
+  unsigned char *ws = nullptr;
+  std::vector<unsigned char> coef_bytes;   // coefficient table in the compute type, for c_coef
+  cudaStream_t last_stream = nullptr;
+  int64_t iters = 0;
+  int sweep_grid = 1, num_sms = 148;
+  int launches_per_iter = 0;
+};
+
+namespace {
+
+template <typename T>
+bte_status launch_skew(bte_solver *h, const double *src, double scale, int which, cudaStream_t st) {
+  const int64_t N = h->pl.dev.ncell;
+  const int grid = (int)std::min<int64_t>((N + 255) / 256, 148 * 16);
+  bte_skew_kernel<T><<<grid, 256, 0, st>>>(h->pl.dev, src, scale, which);
+  CK(cudaGetLastError());
+  return BTE_OK;
+}
+
+bte_status skew(bte_solver *h, const double *src, double scale, int which, cudaStream_t st) {
+  return h->pl.dev.fp32 ? launch_skew<float>(h, src, scale, which, st) : launch_skew<double>(h, src, scale, which, st);
+}
+
+template <typename T>
+bte_status iterate_T(bte_solver *h, int n, cudaStream_t st) {
+  Plan &pl = h->pl;
+  BteDev &dv = pl.dev;
+  CK(cudaMemcpyToSymbolAsync(c_coef, h->coef_bytes.data(), h->coef_bytes.size(), 0, cudaMemcpyHostToDevice, st));
+  const int bgrid = h->num_sms * 4;
+  for (int it = 0; it < n; ++it) {
+    dv.epoch = (int32_t)(h->iters + 1);
+    if (pl.any_diffuse_face) bte_gdiff_kernel<T><<<bgrid, 256, 0, st>>>(dv);
+    bte_ghost_kernel<T><<<bgrid, 256, 0, st>>>(dv);
+    bte_sweep_kernel<T><<<h->sweep_grid, pl.nthreads, pl.smem, st>>>(dv);
+    bte_update_kernel<T><<<dv.n_red_blocks, 256, 0, st>>>(dv);
+    bte_final_kernel<<<1, 256, 0, st>>>(dv);
+    h->iters += 1;
+  }
+  CK(cudaGetLastError());
+  return BTE_OK;
+}
+
+template <typename T>
+bte_status setup_sweep(bte_solver *h) {
+  Plan &pl = h->pl;
+  CK(cudaFuncSetAttribute(bte_sweep_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+  int occ = 0;
+  CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bte_sweep_kernel<T>, pl.nthreads, pl.smem));
+  if (occ < 1) { g_last_cuda = (int)cudaErrorLaunchOutOfResources; return BTE_ERR_CUDA; }
+  h->sweep_grid = (int)std::min<int64_t>(pl.dev.n_units, (int64_t)h->num_sms * occ);
+  return BTE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t bte_workspace_bytes(const bte_problem *p) {
+  Plan pl;
+  if (build_plan(p, pl) != BTE_OK) return 0;
+  return bind(pl, nullptr);
+}
+
+bte_status bte_create(const bte_problem *p, void *d_workspace, size_t bytes, void *cuda_stream, bte_solver **out) {
+  if (!out) return BTE_ERR_INVALID_ARG;
+  bte_solver *h = new (std::nothrow) bte_solver();
+  if (!h) return BTE_ERR_INVALID_ARG;
+  bte_status st = build_plan(p, h->pl);
+  if (st != BTE_OK) { delete h; return st; }
+  const size_t need = bind(h->pl, nullptr);
+  if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255) || bytes < need) { delete h; return BTE_ERR_WORKSPACE; }
+  h->ws = static_cast<unsigned char *>(d_workspace);
+  bind(h->pl, h->ws);
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  Plan &pl = h->pl;
+  BteDev &dv = pl.dev;
+  auto fail = [&](bte_status e) { delete h; return e; };
+#define CKD(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { g_last_cuda = (int)e_; return fail(BTE_ERR_CUDA); } } while (0)
+  int devid = 0;
+  CKD(cudaGetDevice(&devid));
+  CKD(cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, devid));
+  CKD(cudaMemsetAsync(h->ws, 0, need, s));
+  CKD(cudaMemcpyAsync(dv.code, pl.code.data(), pl.code.size(), cudaMemcpyHostToDevice, s));
+  CKD(cudaMemcpyAsync(dv.Qphys, pl.Q.data(), pl.Q.size() * 8, cudaMemcpyHostToDevice, s));
+  if (dv.n_iface) {
+    CKD(cudaMemcpyAsync(dv.iface, pl.iface.data(), pl.iface.size() * 4, cudaMemcpyHostToDevice, s));
+    CKD(cudaMemcpyAsync(dv.iface_info, pl.iface_info.data(), pl.iface_info.size() * 4, cudaMemcpyHostToDevice, s));
+  }
+  CKD(cudaMemcpyAsync((void *)dv.item_coef, pl.item_coef.data(), pl.item_coef.size() * 4, cudaMemcpyHostToDevice, s));
+  CKD(cudaMemcpyAsync(dv.units, pl.units.data(), pl.units.size() * sizeof(BteUnit), cudaMemcpyHostToDevice, s));
+  CKD(cudaMemcpyAsync(dv.band, pl.band.data(), pl.band.size() * 8, cudaMemcpyHostToDevice, s));
+  // coefficient table in the compute type
+  if (dv.fp32) {
+    h->coef_bytes.resize(pl.coef.size() * 4);
+    float *f = reinterpret_cast<float *>(h->coef_bytes.data());
+    for (size_t i = 0; i < pl.coef.size(); ++i) f[i] = (float)pl.coef[i];
+    // unit offsets are in values, identical for both types
+  } else {
+    h->coef_bytes.resize(pl.coef.size() * 8);
+    std::memcpy(h->coef_bytes.data(), pl.coef.data(), pl.coef.size() * 8);
+  }
+  st = dv.fp32 ? setup_sweep<float>(h) : setup_sweep<double>(h);
+  if (st != BTE_OK) return fail(st);
+  st = skew(h, dv.Qphys, 0.0, 2, s);                       // cell codes -> skewed copies
+  if (st == BTE_OK) st = skew(h, dv.Qphys, 1.0 / pl.sumC, 0, s);  // Q / sum C (Eq. 11)
+  if (st != BTE_OK) return fail(st);
+  CKD(cudaStreamSynchronize(s));
+#undef CKD
+  h->last_stream = s;
+  h->launches_per_iter = 4 + (pl.any_diffuse_face ? 1 : 0);
+  *out = h;
+  return BTE_OK;
+}
+
+bte_status bte_iterate(bte_solver *h, int32_t n, void *cuda_stream) {
+  if (!h || n < 0) return BTE_ERR_INVALID_ARG;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  h->last_stream = s;
+  if (n == 0) return BTE_OK;
+  return h->pl.dev.fp32 ? iterate_T<float>(h, n, s) : iterate_T<double>(h, n, s);
+}
+
+bte_status bte_get_temperature(bte_solver *h, double *d_out, void *cuda_stream) {
+  if (!h || !d_out) return BTE_ERR_INVALID_ARG;
+  CK(cudaMemcpyAsync(d_out, h->pl.dev.dT, (size_t)h->pl.dev.ncell * 8, cudaMemcpyDeviceToDevice,
+                     static_cast<cudaStream_t>(cuda_stream)));
+  return BTE_OK;
+}
+
+bte_status bte_get_heat_flux(bte_solver *h, double *d_out, void *cuda_stream) {
+  if (!h || !d_out) return BTE_ERR_INVALID_ARG;
+  CK(cudaMemcpyAsync(d_out, h->pl.dev.q, (size_t)h->pl.dev.ncell * 24, cudaMemcpyDeviceToDevice,
+                     static_cast<cudaStream_t>(cuda_stream)));
+  return BTE_OK;
+}
+
+bte_status bte_set_temperature(bte_solver *h, const double *d_in, void *cuda_stream) {
+  if (!h || !d_in) return BTE_ERR_INVALID_ARG;
+  return skew(h, d_in, 1.0, 1, static_cast<cudaStream_t>(cuda_stream));
+}
+
+bte_status bte_residual(bte_solver *h, double *eps_T, double *eps_q) {
+  if (!h) return BTE_ERR_INVALID_ARG;
+  const double inf = std::numeric_limits<double>::infinity();
+  double eT = inf, eq = inf;
+  if (h->iters > 0) {
+    double r[4];
+    CK(cudaMemcpyAsync(r, h->pl.dev.red + 4 * h->pl.dev.n_red_blocks, 32, cudaMemcpyDeviceToHost, h->last_stream));
+    CK(cudaStreamSynchronize(h->last_stream));
+    const double n = (double)h->pl.dev.nsolid;
+    const double rT = std::sqrt(r[0] / n), rq = std::sqrt(r[2] / n);
+    eT = r[1] > 0 ? rT / r[1] : (rT == 0 ? 0.0 : inf);
+    eq = r[3] > 0 ? rq / r[3] : (rq == 0 ? 0.0 : inf);
+  } else {
+    CK(cudaStreamSynchronize(h->last_stream));
+  }
+  if (eps_T) *eps_T = eT;
+  if (eps_q) *eps_q = eq;
+  return BTE_OK;
+}
+
+bte_status bte_solve_host(bte_solver *h, const double *Q_host, int32_t n, double *dT_host, double *q_host,
+                          void *cuda_stream) {
+  if (!h || n < 0 || !dT_host) return BTE_ERR_INVALID_ARG;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  Plan &pl = h->pl;
+  BteDev &dv = pl.dev;
+  if (Q_host) {
+    CK(cudaMemcpyAsync(dv.Qphys, Q_host, (size_t)dv.ncell * 8, cudaMemcpyHostToDevice, s));
+    bte_status st = skew(h, dv.Qphys, 1.0 / pl.sumC, 0, s);
+    if (st != BTE_OK) return st;
+  }
+  CK(cudaMemsetAsync(h->ws + pl.state_begin, 0, pl.state_end - pl.state_begin, s));
+  h->iters = 0;
+  bte_status st = bte_iterate(h, n, cuda_stream);
+  if (st != BTE_OK) return st;
+  CK(cudaMemcpyAsync(dT_host, dv.dT, (size_t)dv.ncell * 8, cudaMemcpyDeviceToHost, s));
+  if (q_host) CK(cudaMemcpyAsync(q_host, dv.q, (size_t)dv.ncell * 24, cudaMemcpyDeviceToHost, s));
+  CK(cudaStreamSynchronize(s));
+  return BTE_OK;
+}
+
+int64_t bte_updates_per_sweep(const bte_solver *h) {
+  if (!h) return 0;
+  return h->pl.dev.nsolid * h->pl.dev.B * (int64_t)h->pl.dev.n_dirs;
+}
+int64_t bte_iterations_done(const bte_solver *h) { return h ? h->iters : 0; }
+int32_t bte_kernel_launches_per_iteration(const bte_solver *h) { return h ? h->launches_per_iter : 0; }
+
+void bte_schedule_info(const bte_solver *h, int64_t out[6]) {
+  if (!h || !out) return;
+  const Plan &pl = h->pl;
+  out[0] = pl.dev.n_units;
+  out[1] = h->sweep_grid;
+  out[2] = pl.nthreads;
+  out[3] = pl.steps_total;
+  out[4] = pl.steps_total * pl.nthreads * BTE_P;
+  out[5] = (int64_t)pl.total;
+}
+
+void bte_destroy(bte_solver *h) { delete h; }
+
+const char *bte_status_string(bte_status s) {
+  switch (s) {
+    case BTE_OK: return "ok";
+    case BTE_ERR_INVALID_ARG: return "invalid argument";
+    case BTE_ERR_QUADRATURE: return "quadrature rejected";
+    case BTE_ERR_WORKSPACE: return "workspace too small or misaligned";
+    case BTE_ERR_CUDA: return "CUDA error";
+    case BTE_ERR_UNSUPPORTED: return "unsupported problem";
+  }
+  return "unknown";
+}
+int32_t bte_last_cuda_error(void) { return g_last_cuda; }
+
+}  // extern "C"

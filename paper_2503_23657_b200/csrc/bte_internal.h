@@ -35,7 +35,7 @@ struct BteDev {           // passed by value to every kernel
   int32_t nx, ny, nz, dim;
   int32_t nty, ntz, TZ, NU, nyp;    // tiles along y', z'; warps per CTA; nx+31; nty*32
   int32_t B, n_units, has_y, has_z;
-  int32_t nHslot, n_iface, fp32, pad0;
+  int32_t nHslot, n_iface, fp32, n_dirs;
   int64_t NS, ncell, nsolid;
   double inv_sumCtau;
   void *dT_sk[4];         // T  [NS]   lattice temperature deviation, skewed copies per class
@@ -48,6 +48,9 @@ struct BteDev {           // passed by value to every kernel
   void *Gi;               // T  [n_iface][B] interface inflow of this iteration
   double *Hpart;          // [n_iface][B][nHslot] outgoing hemispherical partial sums
   int32_t *iface_info;    // [n_iface] : face code f (0..5)
+  const int32_t *item_coef; // [8][max_items] coefficient-block offset of (octant, item)
+  void *Gf;               // T diffuse box-face inflow [sum_f B*na*nb]
+  int32_t max_items, pad2;
   BteOct oct[8];
   BteUnit *units;
   int32_t *done;          // [n_units] epoch stamps
