@@ -1,0 +1,220 @@
+"""GPU parity: the CUDA path (through the C-ABI of include/bte.h) against the fp64 CPU oracle,
+element by element, on the same seeded inputs after the same iteration count.
+
+Error norms are reading G12: err_T = max|dT_gpu - dT_ref| / max|dT_ref|,
+err_q = max||q_gpu - q_ref||_2 / max||q_ref||_2.  Tolerances are north_star's:
+1e-10 for fp64, 1e-4 for fp32-storage/fp64-accumulate (against the fp64 oracle).
+"""
+import os
+
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = {W.FP64: 1e-10, W.FP32_STORE_FP64_ACC: 1e-4}
+NCPU = max(1, min(32, os.cpu_count() or 1))
+
+
+@pytest.fixture(scope="module")
+def bte():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2503_23657_b200 as m
+    m.lib()          # fails loudly if the in-tree .so is missing
+    return m
+
+
+def errors(dT, q, dT_ref, q_ref):
+    eT = np.max(np.abs(dT - dT_ref)) / max(np.max(np.abs(dT_ref)), 1e-300)
+    dq = np.sqrt(((q - q_ref) ** 2).sum(axis=0))
+    qn = np.sqrt((q_ref ** 2).sum(axis=0))
+    eq = np.max(dq) / max(np.max(qn), 1e-300)
+    return eT, eq
+
+
+def run_both(bte, p, n, precision=None, checkpoints=()):
+    import oracle
+    prec = p.precision if precision is None else precision
+    ref = oracle.RefSolver(p, threads=NCPU)
+    gpu = bte.Solver(p, precision=prec)
+    done = 0
+    out = []
+    for stop in sorted(set(checkpoints) | {n}):
+        ref.iterate(stop - done)
+        gpu.iterate(stop - done)
+        done = stop
+        dT = gpu.temperature().cpu().numpy()
+        q = gpu.heat_flux().cpu().numpy()
+        eT, eq = errors(dT, q, ref.temperature(), ref.heat_flux())
+        rT, rq = ref.residual()
+        gT, gq = gpu.residual()
+        out.append((stop, eT, eq, (rT, rq), (gT, gq)))
+    return out, gpu, ref
+
+
+def check(bte, p, n, precision=None, checkpoints=(), res_rtol=None):
+    prec = p.precision if precision is None else precision
+    tol = TOL[prec]
+    out, gpu, ref = run_both(bte, p, n, prec, checkpoints)
+    for stop, eT, eq, (rT, rq), (gT, gq) in out:
+        assert eT <= tol, f"{p.name} n={stop}: err_T={eT:.3e} > {tol}"
+        assert eq <= tol, f"{p.name} n={stop}: err_q={eq:.3e} > {tol}"
+        # Eq. 23 residuals: same definition on both sides
+        rt = res_rtol if res_rtol is not None else (1e-6 if prec == W.FP64 else 2e-2)
+        if rT > 1e3 * tol and np.isfinite(rT):
+            assert abs(gT - rT) <= rt * rT, f"{p.name} n={stop}: eps_T {gT} vs {rT}"
+        if rq > 1e3 * tol and np.isfinite(rq):
+            assert abs(gq - rq) <= rt * rq, f"{p.name} n={stop}: eps_q {gq} vs {rq}"
+    assert gpu.iterations_done == n
+    assert gpu.updates_per_sweep == p.updates_per_sweep == ref.updates_per_sweep
+    return out
+
+
+# ---------------------------------------------------------------- shrunken configs (T2)
+SHRUNK = {0: (57, 1, 1), 1: (45, 70, 1), 2: (19, 37, 21), 3: (40, 36, 32), 4: (43, 34, 19)}
+
+
+@pytest.mark.parametrize("k", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("prec", [W.FP64, W.FP32_STORE_FP64_ACC])
+def test_shrunken_configs(bte, k, prec):
+    """Every config at a size that spans several tiles with a ragged tail on every axis
+    (tiles are 32 rows in y and 8/16 in z), checked at n = 1, 2, 10, 30."""
+    p = W.config(k, grid=SHRUNK[k])
+    check(bte, p, 30, precision=prec, checkpoints=(1, 2, 10))
+
+
+# ---------------------------------------------------------------- random problems: every BC mix
+@pytest.mark.parametrize("seed", range(8))
+@pytest.mark.parametrize("dim", [1, 2, 3])
+def test_random_masked_problems(bte, seed, dim):
+    p = W.random_problem(seed, dim=dim, shape=(13 + seed, 9 + 5 * (seed % 3), 6 + seed % 4),
+                         masked=(seed % 2 == 0), periodic_axis=(seed % 3 if seed % 4 == 1 else None),
+                         interface_type=(W.BC_DIFFUSE if seed % 3 else W.BC_ISOTHERMAL))
+    check(bte, p, 12, precision=W.FP64, checkpoints=(1, 3))
+    check(bte, p, 12, precision=W.FP32_STORE_FP64_ACC)
+
+
+@pytest.mark.parametrize("bc", [W.BC_ISOTHERMAL, W.BC_DIFFUSE, W.BC_SPECULAR, W.BC_PERIODIC])
+def test_each_bc_type_alone(bte, bc):
+    """One BC type on all side faces, z- isothermal so a steady state exists."""
+    p = W.config(2, grid=(33, 34, 9))
+    fb = [(bc, 0.25 if bc == W.BC_ISOTHERMAL else 0.0)] * 4 + [(W.BC_ISOTHERMAL, -0.3), (W.BC_DIFFUSE, 0.0)]
+    p.face_bc = fb
+    check(bte, p, 15, precision=W.FP64, checkpoints=(1, 2))
+
+
+def test_periodic_wrap_onto_void_uses_interface_bc(bte):
+    """Reading: a periodic wrap that lands on a void cell falls through to interface_bc."""
+    p = W.config(3, grid=(12, 20, 16))
+    p.mask = p.mask.copy()
+    p.mask[:, :, 0] = 0          # x=0 plane void: wrap from x=nx-1 hits void
+    p.mask[0, 0, 0] = 1
+    p.Q = p.Q * p.mask
+    check(bte, p, 10, precision=W.FP64, checkpoints=(1,))
+
+
+# ---------------------------------------------------------------- edge cases
+def test_single_cell_and_tiny_grids(bte):
+    for shape, dim in [((1, 1, 1), 1), ((1, 1, 1), 3), ((2, 1, 1), 2), ((1, 3, 2), 3), ((3, 1, 1), 1)]:
+        p = W.random_problem(3, dim=dim, shape=shape, masked=False)
+        check(bte, p, 6, precision=W.FP64, checkpoints=(1,))
+
+
+def test_zero_iterations_and_zero_source(bte):
+    p = W.config(2, grid=(9, 8, 7))
+    g = bte.Solver(p)
+    g.iterate(0)
+    assert g.iterations_done == 0
+    assert float(g.temperature().abs().max()) == 0.0
+    eT, eq = g.residual()
+    assert np.isinf(eT) and np.isinf(eq)
+    p.Q = None
+    p.face_bc = [(W.BC_DIFFUSE, 0.0)] * 4 + [(W.BC_ISOTHERMAL, 0.0), (W.BC_DIFFUSE, 0.0)]
+    g = bte.Solver(p)
+    g.iterate(3)
+    assert float(g.temperature().abs().max()) == 0.0
+    assert g.residual() == (0.0, 0.0)          # 0/0 -> 0 (reading G11)
+
+
+def test_set_temperature_restart(bte):
+    import oracle
+    p = W.config(2, grid=(17, 9, 11))
+    rng = np.random.default_rng(7)
+    dT0 = rng.uniform(-1, 1, size=(p.nz, p.ny, p.nx))
+    ref = oracle.RefSolver(p); ref.set_temperature(dT0); ref.iterate(1)
+    g = bte.Solver(p); g.set_temperature(dT0); g.iterate(1)
+    eT, eq = errors(g.temperature().cpu().numpy(), g.heat_flux().cpu().numpy(), ref.temperature(), ref.heat_flux())
+    assert eT <= 1e-10 and eq <= 1e-10
+
+
+def test_bitwise_deterministic(bte):
+    p = W.config(3, grid=(24, 40, 24))
+    a = bte.Solver(p); a.iterate(7)
+    b = bte.Solver(p); b.iterate(3); b.iterate(4)
+    assert (a.temperature() == b.temperature()).all()
+    assert (a.heat_flux() == b.heat_flux()).all()
+
+
+def test_solve_host_matches_device_path(bte):
+    p = W.config(2, grid=(20, 12, 9))
+    g = bte.Solver(p); g.iterate(5)
+    h = bte.Solver(p)
+    dT, q = h.solve_host(np.ascontiguousarray(p.Q), 5)
+    assert (dT == g.temperature().cpu().numpy()).all()
+    assert (q == g.heat_flux().cpu().numpy()).all()
+    dT2, _ = h.solve_host(None, 5)      # state is reset on every call
+    assert (dT2 == dT).all()
+
+
+def test_non_default_stream(bte):
+    import torch
+    p = W.config(1, grid=(40, 33, 1))
+    a = bte.Solver(p); a.iterate(4)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        b = bte.Solver(p); b.iterate(4); t = b.temperature()
+    s.synchronize()
+    assert (a.temperature() == t).all()
+
+
+# ---------------------------------------------------------------- full sizes (T3)
+def test_config0_full_matches_oracle_and_golden(bte):
+    p = W.config(0)
+    check(bte, p, p.n_iter, checkpoints=(1, 10, 35))
+    gold = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "cfg0_kn1_film.txt"))
+    g = bte.Solver(p); g.iterate(p.n_iter)
+    dT = g.temperature().cpu().numpy().ravel()
+    qx = g.heat_flux().cpu().numpy()[0].ravel()
+    assert np.max(np.abs(dT - gold[:, 1])) <= 1e-10 * np.max(np.abs(gold[:, 1]))
+    assert np.max(np.abs(qx - gold[:, 2])) <= 1e-10 * np.max(np.abs(gold[:, 2]))
+
+
+@pytest.mark.slow
+def test_config1_full(bte):
+    p = W.config(1)
+    check(bte, p, 20, checkpoints=(1,))
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("prec", [W.FP64, W.FP32_STORE_FP64_ACC])
+def test_config2_full(bte, prec):
+    p = W.config(2)
+    check(bte, p, 6, precision=prec, checkpoints=(1,))
+
+
+@pytest.mark.slow
+def test_config3_full(bte):
+    p = W.config(3)
+    check(bte, p, 5, checkpoints=(1,))
+
+
+@pytest.mark.slow
+def test_config4_full_sampled(bte):
+    """Full-size config 4 in the launch configuration bench.py times: 2 iterations against the
+    (multi-threaded, bit-identical) oracle on every cell, plus size-independent properties."""
+    p = W.config(4)
+    out = check(bte, p, 2, checkpoints=(1,))
+    assert out[-1][1] <= 1e-4
