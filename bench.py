@@ -1,0 +1,249 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line with the headline metric of BASELINE.json:
+band*dir*cell updates/s per sweep (whole source iterations: sweep + moments + dT/q/residual update).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+A "step" is one source iteration of the whole hot path on one seeded
+synthetic problem (workloads.config(k)).  N > 1 (torchrun): replicas only -- every rank runs an
+independent copy of the problem, value = sum of updates / max-over-ranks time.
+`--impl reference` times the CPU oracle as it stands on the host cores (rank 0 only).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "band*dir*cell updates/s per sweep"
+UNIT = "updates/s"
+FLOP_PER_UPDATE = 16.0        # 3 FMA + 1 MUL (recurrence) + 4 FMA (moments), SURVEY.md 8(a)/DESIGN.md
+SM_COUNT, SM_MAX_HZ = 148, 1.965e9
+# plain-ALU peaks derived from unit counts x max clock: FP32 128 FMA/clk/SM,
+# FP64 64 FMA/clk/SM
+PEAK_TFLOPS = {"f32": SM_COUNT * 128 * 2 * SM_MAX_HZ / 1e12, "f64": SM_COUNT * 64 * 2 * SM_MAX_HZ / 1e12}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs[k]")
+    ap.add_argument("--precision", choices=["config", "f64", "f32"], default="config")
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--converge", action="store_true", help="also report time to eps_T <= 1e-8")
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm = sorted(int(r[0]) for r in self.rows if r and r[0].isdigit())
+        mx = [int(r[1]) for r in self.rows if len(r) > 1 and r[1].isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(len(r) > 2 + k and r[2 + k] == "Active" for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def oracle_sample(W, k, budget_s, steps):
+    """Pick the largest replica of config k (same physical size, coarser grid) whose `steps` oracle
+    iterations fit `budget_s` on this host; the oracle runs threaded over bands (bit-identical)."""
+    cores = max(1, min(os.cpu_count() or 1, 15))
+    full = W.config(k)
+    grids = [(full.nx, full.ny, full.nz)]
+    while max(grids[-1]) > 8:
+        g = grids[-1]
+        grids.append((max(g[0] // 2, 1), max(g[1] // 2, 1) if full.dim > 1 else 1, max(g[2] // 2, 1) if full.dim > 2 else 1))
+    rate = 2.0e7 * cores                      # conservative guess [updates/s]; only sizes the sample
+    for g in grids:
+        p = W.config(k, grid=g)
+        if p.updates_per_sweep * steps / rate <= budget_s:
+            return p, g, cores
+    return p, g, cores
+
+
+def time_oracle(W, k, budget_s, steps=1, warmup=0):
+    import oracle
+    p, grid, cores = oracle_sample(W, k, budget_s, steps + warmup)
+    r = oracle.RefSolver(p, threads=cores)
+    r.iterate(warmup)
+    t0 = time.perf_counter()
+    r.iterate(steps)
+    dt = time.perf_counter() - t0
+    return {"value": p.updates_per_sweep * steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{steps} source iteration(s) of config {k} on a {grid[0]}x{grid[1]}x{grid[2]} replica "
+                      f"({p.updates_per_sweep:.3e} updates each), oracle threaded over bands"}, dt / steps, p
+
+
+def run_reference(args, W):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cb, s_per_step, p = time_oracle(W, args.config, budget_s=150.0, steps=args.steps, warmup=args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": s_per_step * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"configs[{args.config}] {p.name} (bounded sample, see cpu_baseline.sample)",
+                       "grid": [p.nx, p.ny, p.nz], "bands": len(p.C), "directions": len(p.w)},
+            "cpu_baseline": cb,
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, W):
+    import torch
+    import torch.distributed as dist
+    import paper_2503_23657_b200 as bte
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    p = W.config(args.config)
+    prec = {"config": p.precision, "f64": W.FP64, "f32": W.FP32_STORE_FP64_ACC}[args.precision]
+    dtype = "f32" if prec == W.FP32_STORE_FP64_ACC else "f64"
+    solver = bte.Solver(p, precision=prec, device=dev)
+    K, Wm = args.steps, max(args.warmup, 3)
+    upd = solver.updates_per_sweep
+
+    # ---- device-resident timing: K iterations in one bte_iterate call (inputs already in HBM)
+    solver.iterate(Wm)
+    solver.set_sweep_timing(K)
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    solver.iterate(K)
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms = float(ms.item())
+    sweep_ms, sweep_n = solver.sweep_timing()
+    solver.set_sweep_timing(0)
+    eps = solver.residual()
+
+    # ---- end to end through the C-ABI host-buffer call: every step uploads Q from pinned host memory,
+    # runs one iteration and downloads dT into pinned host memory
+    Qh = torch.from_numpy(p.Q.astype("float64")).contiguous().pin_memory()
+    dTh = torch.empty(solver.shape, dtype=torch.float64).pin_memory()
+    for _ in range(3):
+        solver.solve_host(Qh, 1, reset=False, out=(dTh, None))
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        solver.solve_host(Qh, 1, reset=False, out=(dTh, None))
+    barrier()
+    e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    e2e_s = float(e2e_s.item())
+
+    conv = None
+    if args.converge and rank == 0:
+        solver.solve_host(Qh, 0, reset=True, out=(dTh, None))
+        torch.cuda.synchronize()
+        t0, n = time.perf_counter(), 0
+        while n < 20000:
+            solver.iterate(25)
+            n += 25
+            if solver.residual()[0] <= 1e-8:
+                break
+        conv = {"eps_T_target": 1e-8, "iterations": n, "seconds": time.perf_counter() - t0,
+                "eps_T": solver.residual()[0]}
+
+    if rank == 0:
+        sweep_avg_ms = sweep_ms / max(sweep_n, 1)
+        achieved = upd * FLOP_PER_UPDATE / (sweep_avg_ms * 1e-3) / 1e12
+        peak = PEAK_TFLOPS[dtype]
+        info = solver.schedule_info()
+        line = {"metric": METRIC, "value": world * upd * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+                "steps": K, "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": dtype, "data": "synthetic",
+                "config": {"workload": f"configs[{args.config}] {p.name}", "grid": [p.nx, p.ny, p.nz],
+                           "solid_cells": p.n_solid, "bands": len(p.C), "directions": len(p.w),
+                           "updates_per_step": upd, "parallelism": "replicas" if world > 1 else "single",
+                           "l2": f"working set {info['workspace_bytes'] / 1e6:.0f} MB > 126 MB L2 (no flush needed)"
+                                 if info["workspace_bytes"] > 2 * 126e6 else "working set fits L2 (state is L2-resident by design)",
+                           "eps_T_after_timed_steps": eps[0]},
+                "clocks": clocks,
+                "e2e": {"value": world * upd * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": Qh.numel() * 8,
+                        "d2h_bytes_per_step": dTh.numel() * 8,
+                        "what": "bte_solve_host(Q pinned host -> 1 iteration -> dT pinned host) per step"},
+                "gpu_launches": solver.launches_per_iteration * K,
+                "roofline": {"bound": "alu", "kernel": "bte_sweep_kernel", "achieved": achieved, "peak": peak,
+                             "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                             "peak_source": "derived: 148 SMs x %d FMA/clk x 2 x 1.965 GHz (DESIGN.md)" % (128 if dtype == "f32" else 64),
+                             "ms_per_launch": sweep_avg_ms, "launches_timed": sweep_n,
+                             "share_of_step": sweep_ms / ms if ms > 0 else None,
+                             "wavefront_occupancy": upd / info["thread_slot_updates"]},
+                }
+        if conv:
+            line["time_to_1e-8"] = conv
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = time_oracle(W, args.config, budget_s=20.0, steps=1)[0]
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    import workloads as W
+    if args.impl == "reference":
+        run_reference(args, W)
+    else:
+        run_ours(args, W)
+
+
+if __name__ == "__main__":
+    main()

@@ -101,10 +101,17 @@ bte_status bte_set_temperature(bte_solver *h, const double *d_in, void *cuda_str
 bte_status bte_residual(bte_solver *h, double *eps_T, double *eps_q);
 
 /* Whole-path convenience with HOST buffers (used for end-to-end timing): uploads Q (host, [nx*ny*nz],
- * may be NULL = keep), resets dT and the store to 0, runs n iterations, downloads dT (host [nx*ny*nz])
- * and q (host [3][nx*ny*nz]; may be NULL). Synchronous. */
-bte_status bte_solve_host(bte_solver *h, const double *Q_host, int32_t n, double *dT_host, double *q_host,
-                          void *cuda_stream);
+ * may be NULL = keep); if reset != 0 sets dT and the lagged store back to 0 and the iteration count to 0;
+ * runs n iterations; downloads dT (host [nx*ny*nz]) and q (host [3][nx*ny*nz]; may be NULL).
+ * Synchronous (returns after the downloads completed). */
+bte_status bte_solve_host(bte_solver *h, const double *Q_host, int32_t n, int32_t reset, double *dT_host,
+                          double *q_host, void *cuda_stream);
+
+/* Measurement aid: record a CUDA-event pair around the sweep kernel of the next max_launches iterations
+ * (on the stream bte_iterate is given); 0 switches it off. bte_get_sweep_timing synchronises on the last
+ * recorded event, returns the summed device time [ms] and the number of launches covered, and re-arms. */
+bte_status bte_set_sweep_timing(bte_solver *h, int32_t max_launches);
+bte_status bte_get_sweep_timing(bte_solver *h, double *total_ms, int64_t *launches);
 
 int64_t bte_updates_per_sweep(const bte_solver *h); /* solid cells * n_bands * n_dirs */
 int64_t bte_iterations_done(const bte_solver *h);

@@ -30,7 +30,8 @@ STATUS = {0: "BTE_OK", 1: "BTE_ERR_INVALID_ARG", 2: "BTE_ERR_QUADRATURE", 3: "BT
 BTE_FP64, BTE_FP32_STORE_FP64_ACC = 0, 1
 
 EXPORTS = ["bte_workspace_bytes", "bte_create", "bte_iterate", "bte_get_temperature", "bte_get_heat_flux",
-           "bte_set_temperature", "bte_residual", "bte_solve_host", "bte_updates_per_sweep",
+           "bte_set_temperature", "bte_residual", "bte_solve_host", "bte_set_sweep_timing",
+           "bte_get_sweep_timing", "bte_updates_per_sweep",
            "bte_iterations_done", "bte_kernel_launches_per_iteration", "bte_schedule_info", "bte_destroy",
            "bte_status_string", "bte_last_cuda_error"]
 
@@ -89,7 +90,9 @@ def lib():
         L.bte_get_heat_flux.argtypes = [vp, vp, vp]
         L.bte_set_temperature.argtypes = [vp, vp, vp]
         L.bte_residual.argtypes = [vp, dp, dp]
-        L.bte_solve_host.argtypes = [vp, vp, i32, vp, vp, vp]
+        L.bte_solve_host.argtypes = [vp, vp, i32, i32, vp, vp, vp]
+        L.bte_set_sweep_timing.argtypes = [vp, i32]
+        L.bte_get_sweep_timing.argtypes = [vp, dp, C.POINTER(i64)]
         L.bte_updates_per_sweep.argtypes = [vp]
         L.bte_updates_per_sweep.restype = i64
         L.bte_iterations_done.argtypes = [vp]
@@ -206,16 +209,33 @@ class Solver:
             raise BteError(rc, "bte_residual")
         return a.value, b.value
 
-    def solve_host(self, Q_host, n, want_q=True, stream=None):
-        """End-to-end call with HOST buffers (numpy / pinned torch CPU tensors)."""
-        dT = np.empty(self.shape, dtype=np.float64)
-        q = np.empty((3,) + self.shape, dtype=np.float64) if want_q else None
-        qp = None if Q_host is None else C.c_void_p(Q_host.ctypes.data if isinstance(Q_host, np.ndarray) else Q_host.data_ptr())
-        rc = lib().bte_solve_host(self.h, qp, int(n), C.c_void_p(dT.ctypes.data),
-                                  None if q is None else C.c_void_p(q.ctypes.data), self._stream(stream))
+    def solve_host(self, Q_host, n, want_q=True, reset=True, out=None, stream=None):
+        """End-to-end call with HOST buffers (numpy arrays or pinned torch CPU tensors).
+        `out` = (dT, q) preallocated host buffers (q may be None) to avoid allocation in timed loops."""
+        ptr = lambda a: C.c_void_p(a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr())
+        if out is None:
+            dT = np.empty(self.shape, dtype=np.float64)
+            q = np.empty((3,) + self.shape, dtype=np.float64) if want_q else None
+        else:
+            dT, q = out
+        rc = lib().bte_solve_host(self.h, None if Q_host is None else ptr(Q_host), int(n), int(bool(reset)),
+                                  ptr(dT), None if q is None else ptr(q), self._stream(stream))
         if rc:
             raise BteError(rc, "bte_solve_host")
         return dT, q
+
+    def set_sweep_timing(self, max_launches):
+        rc = lib().bte_set_sweep_timing(self.h, int(max_launches))
+        if rc:
+            raise BteError(rc, "bte_set_sweep_timing")
+
+    def sweep_timing(self):
+        """(summed sweep-kernel device time [ms], launches covered) since the last call."""
+        ms, n = C.c_double(), C.c_int64()
+        rc = lib().bte_get_sweep_timing(self.h, C.byref(ms), C.byref(n))
+        if rc:
+            raise BteError(rc, "bte_get_sweep_timing")
+        return ms.value, n.value
 
     @property
     def updates_per_sweep(self):

@@ -322,6 +322,10 @@ struct bte_solver {
   int64_t iters = 0;
   int sweep_grid = 1, num_sms = 148;
   int launches_per_iter = 0;
+  // optional device timing of the sweep kernel (bte_set_sweep_timing)
+  bool timing = false;
+  std::vector<cudaEvent_t> ev;             // pairs (start, stop)
+  size_t ev_used = 0;
 };
 
 namespace {
@@ -349,7 +353,10 @@ bte_status iterate_T(bte_solver *h, int n, cudaStream_t st) {
     dv.epoch = (int32_t)(h->iters + 1);
     if (pl.any_diffuse_face) bte_gdiff_kernel<T><<<bgrid, 256, 0, st>>>(dv);
     bte_ghost_kernel<T><<<bgrid, 256, 0, st>>>(dv);
+    const bool tm = h->timing && h->ev_used + 2 <= h->ev.size();
+    if (tm) CK(cudaEventRecord(h->ev[h->ev_used], st));
     bte_sweep_kernel<T><<<h->sweep_grid, pl.nthreads, pl.smem, st>>>(dv);
+    if (tm) { CK(cudaEventRecord(h->ev[h->ev_used + 1], st)); h->ev_used += 2; }
     bte_update_kernel<T><<<dv.n_red_blocks, 256, 0, st>>>(dv);
     bte_final_kernel<<<1, 256, 0, st>>>(dv);
     h->iters += 1;
@@ -477,8 +484,35 @@ bte_status bte_residual(bte_solver *h, double *eps_T, double *eps_q) {
   return BTE_OK;
 }
 
-bte_status bte_solve_host(bte_solver *h, const double *Q_host, int32_t n, double *dT_host, double *q_host,
-                          void *cuda_stream) {
+bte_status bte_set_sweep_timing(bte_solver *h, int32_t max_launches) {
+  if (!h || max_launches < 0 || max_launches > 4096) return BTE_ERR_INVALID_ARG;
+  for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
+  h->ev.clear(); h->ev_used = 0; h->timing = max_launches > 0;
+  for (int i = 0; i < 2 * max_launches; ++i) {
+    cudaEvent_t e;
+    CK(cudaEventCreate(&e));
+    h->ev.push_back(e);
+  }
+  return BTE_OK;
+}
+
+bte_status bte_get_sweep_timing(bte_solver *h, double *total_ms, int64_t *launches) {
+  if (!h) return BTE_ERR_INVALID_ARG;
+  double tot = 0;
+  if (h->ev_used) CK(cudaEventSynchronize(h->ev[h->ev_used - 1]));
+  for (size_t i = 0; i + 1 < h->ev_used; i += 2) {
+    float ms = 0;
+    CK(cudaEventElapsedTime(&ms, h->ev[i], h->ev[i + 1]));
+    tot += ms;
+  }
+  if (total_ms) *total_ms = tot;
+  if (launches) *launches = (int64_t)(h->ev_used / 2);
+  h->ev_used = 0;
+  return BTE_OK;
+}
+
+bte_status bte_solve_host(bte_solver *h, const double *Q_host, int32_t n, int32_t reset, double *dT_host,
+                          double *q_host, void *cuda_stream) {
   if (!h || n < 0 || !dT_host) return BTE_ERR_INVALID_ARG;
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   Plan &pl = h->pl;
@@ -488,8 +522,10 @@ bte_status bte_solve_host(bte_solver *h, const double *Q_host, int32_t n, double
     bte_status st = skew(h, dv.Qphys, 1.0 / pl.sumC, 0, s);
     if (st != BTE_OK) return st;
   }
-  CK(cudaMemsetAsync(h->ws + pl.state_begin, 0, pl.state_end - pl.state_begin, s));
-  h->iters = 0;
+  if (reset) {
+    CK(cudaMemsetAsync(h->ws + pl.state_begin, 0, pl.state_end - pl.state_begin, s));
+    h->iters = 0;
+  }
   bte_status st = bte_iterate(h, n, cuda_stream);
   if (st != BTE_OK) return st;
   CK(cudaMemcpyAsync(dT_host, dv.dT, (size_t)dv.ncell * 8, cudaMemcpyDeviceToHost, s));
@@ -516,7 +552,11 @@ void bte_schedule_info(const bte_solver *h, int64_t out[6]) {
   out[5] = (int64_t)pl.total;
 }
 
-void bte_destroy(bte_solver *h) { delete h; }
+void bte_destroy(bte_solver *h) {
+  if (!h) return;
+  for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
+  delete h;
+}
 
 const char *bte_status_string(bte_status s) {
   switch (s) {
