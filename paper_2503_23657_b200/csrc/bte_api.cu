@@ -43,6 +43,14 @@ struct Plan {
   size_t total = 0, state_begin = 0, state_end = 0;
   bool any_diffuse_face = false;
   size_t gf_elems = 0;
+  // fast path (bte_sweep2.cuh)
+  bool v2 = false;
+  Bte2Dev d2{};
+  std::vector<Bte2Unit> units2;
+  Bte2Coefs<float> cf32{};
+  Bte2Coefs<double> cf64{};
+  size_t smem2 = 0;
+  size_t x2_chunks = 0, y2_chunks = 0, z2_chunks = 0;
   size_t xpl_elems[8]{}, ypl_elems[8]{}, zpl_elems[8]{};
 };
 
@@ -268,6 +276,70 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
     pl.zpl_elems[o] = dv.has_z ? (size_t)(dv.ntz + 1) * O.nitems * dv.nty * dv.NU * BTE_P * 32 : 0;
   }
   dv.n_red_blocks = (int)std::min<int64_t>((N + 255) / 256, 148 * 8);
+
+  // ---- fast path: 3-D, all solid, 16 directions in each of the 8 octants with identical |s|, w tables
+  // (mirror-symmetric quadrature), <= 16 bands.  Anything else runs the generic kernels above.
+  bool v2 = p->dim == 3 && nif == 0 && nsolid == N && B <= BTE2_MAXB && p->nx <= 60000;
+  if (const char *e = std::getenv("BTE_FORCE_GENERIC")) if (e[0] == '1') v2 = false;
+  for (int o = 0; o < 8 && v2; ++o) {
+    if ((int)od[o].size() != BTE2_P) v2 = false;
+    for (int b = 0; b < B && v2; ++b)
+      if (pl.item_coef[(size_t)o * max_items + b] != pl.item_coef[b]) v2 = false;
+  }
+  pl.v2 = v2;
+  if (v2) {
+    Bte2Dev &d = pl.d2;
+    int W = p->nz >= 48 ? 8 : 4;
+    if (const char *e = std::getenv("BTE_V2_W")) { const int w = std::atoi(e); if (w == 4 || w == 8) W = w; }
+    d.nx = p->nx; d.ny = p->ny; d.nz = p->nz; d.B = B; d.W = W;
+    d.nty = (p->ny + 63) / 64; d.ntz = (p->nz + 2 * W - 1) / (2 * W); d.NU = p->nx + 31;
+    d.nsteps = p->nx + 31 + W - 1;
+    d.NS = (int64_t)p->nz * d.nty * d.NU * 64;
+    d.ncell = N; d.inv_sumCtau = dv.inv_sumCtau;
+    const int NBmax = dv.fp32 ? 2 : 1, G = (B + NBmax - 1) / NBmax;
+    for (int b = 0; b < B; ++b) {
+      const double *blk = pl.coef.data() + pl.item_coef[b];
+      for (int q = 0; q < BTE2_P; ++q) {
+        const double *r = blk + q * BTE_NCOEF;
+        double k[8] = {r[0], r[1], r[2], r[3], r[4] / p->tau[b], p->v[b] * r[5], p->v[b] * r[6], p->v[b] * r[7]};
+        for (int c = 0; c < 8; ++c) { pl.cf64.k[b][q][c] = k[c]; pl.cf32.k[b][q][c] = (float)k[c]; }
+        if (b == 0) for (int a = 0; a < 3; ++a) d.wsa[q][a] = r[5 + a];
+      }
+      pl.cf64.bc[b][0] = pl.band[b]; pl.cf64.bc[b][1] = pl.band[B + b];
+      pl.cf32.bc[b][0] = (float)pl.band[b]; pl.cf32.bc[b][1] = (float)pl.band[B + b];
+    }
+    for (int f = 0; f < 6; ++f) {
+      d.face_type[f] = dv.face_type[f]; d.Pi_face[f] = dv.Pi_face[f];
+      for (int b = 0; b < B; ++b) d.face_e0[f][b] = pl.band[b] * dv.face_dT[f];
+    }
+    for (int o = 0; o < 8; ++o) {
+      d.oct[o].sx = (o & 1) ? -1 : 1; d.oct[o].sy = (o & 2) ? -1 : 1; d.oct[o].sz = (o & 4) ? -1 : 1;
+      d.oct[o].cls = o & 3;
+    }
+    // units in ticket order (g, ty, tz, octant): every dependency has a smaller index
+    auto uid = [&](int g, int ty, int tz, int o) { return ((g * d.nty + ty) * d.ntz + tz) * 8 + o; };
+    pl.units2.resize((size_t)G * d.nty * d.ntz * 8);
+    for (int g = 0; g < G; ++g) for (int ty = 0; ty < d.nty; ++ty) for (int tz = 0; tz < d.ntz; ++tz) for (int o = 0; o < 8; ++o) {
+      Bte2Unit &U = pl.units2[uid(g, ty, tz, o)];
+      U.oct = o; U.g = g; U.ty = ty; U.tz = tz;
+      U.dep_y = ty > 0 ? uid(g, ty - 1, tz, o) : -1;
+      U.dep_z = tz > 0 ? uid(g, ty, tz - 1, o) : -1;
+      U.dep_prev = g > 0 ? uid(g - 1, ty, tz, o) : -1;
+      U.b0 = g * NBmax; U.nb = std::min(NBmax, B - U.b0);
+    }
+    d.n_units = (int32_t)pl.units2.size();
+    const size_t nch = BTE2_P * tsz / 16;
+    pl.x2_chunks = (size_t)d.ntz * d.nty * B * W * 2 * 2 * nch * 32;
+    pl.y2_chunks = (size_t)(d.nty + 1) * d.ntz * B * W * d.nx * 2 * nch;
+    pl.z2_chunks = (size_t)(d.ntz + 1) * d.nty * B * d.NU * 2 * nch * 32;
+    int64_t off = 0;
+    for (int f = 0; f < 6; ++f) {
+      const int a = f >> 1;
+      const int64_t na = a == 0 ? p->ny : p->nx, nb = a == 2 ? p->ny : p->nz;
+      d.gf_off[f] = off; off += na * nb * B;
+    }
+    pl.steps_total = (int64_t)pl.units2.size() * d.nsteps;
+  }
   return BTE_OK;
 }
 
@@ -279,11 +351,36 @@ size_t bind(Plan &pl, unsigned char *ws) {
   auto take = [&](size_t bytes) { void *p = ws ? ws + off : nullptr; off = align_up(off + bytes); return p; };
   const size_t N = (size_t)dv.ncell, NS = (size_t)dv.NS;
   dv.code = (uint8_t *)take(N);
-  for (int c = 0; c < 4; ++c) dv.code_sk[c] = (uint8_t *)take(NS);
-  for (int c = 0; c < 4; ++c) dv.Q_sk[c] = take(NS * tsz);
   dv.Qphys = (double *)take(N * 8);
-  dv.iface = dv.n_iface ? (int32_t *)take((size_t)6 * N * 4) : nullptr;
-  dv.iface_info = dv.n_iface ? (int32_t *)take((size_t)dv.n_iface * 4) : nullptr;
+  if (!pl.v2) {
+    for (int c = 0; c < 4; ++c) dv.code_sk[c] = (uint8_t *)take(NS);
+    for (int c = 0; c < 4; ++c) dv.Q_sk[c] = take(NS * tsz);
+    dv.iface = dv.n_iface ? (int32_t *)take((size_t)6 * N * 4) : nullptr;
+    dv.iface_info = dv.n_iface ? (int32_t *)take((size_t)dv.n_iface * 4) : nullptr;
+  }
+  if (pl.v2) {
+    Bte2Dev &d = pl.d2;
+    const size_t NS2 = (size_t)d.NS;
+    d.units = (const Bte2Unit *)take(pl.units2.size() * sizeof(Bte2Unit));
+    pl.state_begin = off;
+    d.prog = (int32_t *)take((size_t)d.n_units * 4);
+    d.ticket = (int32_t *)take(256);
+    dv.red = (double *)take((size_t)(4 * dv.n_red_blocks + 4) * 8);
+    dv.dT = (double *)take(N * 8);
+    dv.q = (double *)take(3 * N * 8);
+    dv.qmag = (double *)take(N * 8);
+    d.Gf = take(std::max<size_t>(pl.gf_elems, 1) * tsz);
+    for (int o = 0; o < 8; ++o) {
+      d.oct[o].M = take(NS2 * 4 * tsz);
+      d.oct[o].xin = take(pl.x2_chunks * 16); d.oct[o].xout = take(pl.x2_chunks * 16);
+      d.oct[o].ypl = take(pl.y2_chunks * 16); d.oct[o].zpl = take(pl.z2_chunks * 16);
+    }
+    pl.state_end = off;
+    for (int c = 0; c < 4; ++c) d.dTQ[c] = take(NS2 * 2 * tsz);
+    d.dT = dv.dT; d.q = dv.q; d.qmag = dv.qmag; d.red = dv.red; d.n_red_blocks = dv.n_red_blocks;
+    pl.total = off;
+    return off;
+  }
   dv.item_coef = (const int32_t *)take((size_t)8 * dv.max_items * 4);
   dv.units = (BteUnit *)take((size_t)dv.n_units * sizeof(BteUnit));
   dv.band = (double *)take((size_t)4 * dv.B * 8);
@@ -339,8 +436,66 @@ bte_status launch_skew(bte_solver *h, const double *src, double scale, int which
   return BTE_OK;
 }
 
+template <typename T>
+bte_status launch_skew2(bte_solver *h, const double *src, double scale, int which, cudaStream_t st) {
+  const int64_t N = h->pl.dev.ncell;
+  const int grid = (int)std::min<int64_t>((N + 255) / 256, 148 * 16);
+  bte2_skew_kernel<T><<<grid, 256, 0, st>>>(h->pl.d2, src, scale, which);
+  CK(cudaGetLastError());
+  return BTE_OK;
+}
+
 bte_status skew(bte_solver *h, const double *src, double scale, int which, cudaStream_t st) {
+  if (h->pl.v2) {
+    if (which == 2) return BTE_OK;   // no cell codes on the fast path
+    return h->pl.dev.fp32 ? launch_skew2<float>(h, src, scale, which, st) : launch_skew2<double>(h, src, scale, which, st);
+  }
   return h->pl.dev.fp32 ? launch_skew<float>(h, src, scale, which, st) : launch_skew<double>(h, src, scale, which, st);
+}
+
+template <typename T, int W>
+void launch_sweep2(bte_solver *h, const Bte2Coefs<T> &cf, cudaStream_t st) {
+  bte2_sweep_kernel<T, W><<<h->sweep_grid, W * 32, h->pl.smem2, st>>>(h->pl.d2, cf);
+}
+
+template <typename T>
+bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t st) {
+  Plan &pl = h->pl;
+  Bte2Dev &d = pl.d2;
+  const int bgrid = h->num_sms * 8;
+  for (int it = 0; it < n; ++it) {
+    const int ep = (int)(h->iters % 30000) + 1;
+    if (ep == 1 && h->iters > 0) CK(cudaMemsetAsync(d.prog, 0, (size_t)d.n_units * 4, st));
+    d.epoch = ep;
+    if (pl.any_diffuse_face) bte2_gdiff_kernel<T><<<bgrid, 256, 0, st>>>(d);
+    bte2_ghost_kernel<T><<<bgrid, 256, 0, st>>>(d);
+    const bool tm = h->timing && h->ev_used + 2 <= h->ev.size();
+    if (tm) CK(cudaEventRecord(h->ev[h->ev_used], st));
+    if (d.W == 8) launch_sweep2<T, 8>(h, cf, st); else launch_sweep2<T, 4>(h, cf, st);
+    if (tm) { CK(cudaEventRecord(h->ev[h->ev_used + 1], st)); h->ev_used += 2; }
+    bte2_update_kernel<T><<<pl.dev.n_red_blocks, 256, 0, st>>>(d);
+    bte_final_kernel<<<1, 256, 0, st>>>(pl.dev);
+    h->iters += 1;
+  }
+  CK(cudaGetLastError());
+  return BTE_OK;
+}
+
+template <typename T, int W>
+bte_status setup_sweep2_W(bte_solver *h) {
+  Plan &pl = h->pl;
+  pl.smem2 = sizeof(Bte2Smem<T, sizeof(T) == 4 ? 2 : 1, W>);
+  CK(cudaFuncSetAttribute(bte2_sweep_kernel<T, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem2));
+  int occ = 0;
+  CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bte2_sweep_kernel<T, W>, W * 32, pl.smem2));
+  if (occ < 1) { g_last_cuda = (int)cudaErrorLaunchOutOfResources; return BTE_ERR_CUDA; }
+  h->sweep_grid = (int)std::min<int64_t>(pl.d2.n_units, (int64_t)h->num_sms * occ);
+  pl.nthreads = W * 32;
+  return BTE_OK;
+}
+template <typename T>
+bte_status setup_sweep2(bte_solver *h) {
+  return h->pl.d2.W == 8 ? setup_sweep2_W<T, 8>(h) : setup_sweep2_W<T, 4>(h);
 }
 
 template <typename T>
@@ -407,13 +562,17 @@ bte_status bte_create(const bte_problem *p, void *d_workspace, size_t bytes, voi
   CKD(cudaMemsetAsync(h->ws, 0, need, s));
   CKD(cudaMemcpyAsync(dv.code, pl.code.data(), pl.code.size(), cudaMemcpyHostToDevice, s));
   CKD(cudaMemcpyAsync(dv.Qphys, pl.Q.data(), pl.Q.size() * 8, cudaMemcpyHostToDevice, s));
-  if (dv.n_iface) {
-    CKD(cudaMemcpyAsync(dv.iface, pl.iface.data(), pl.iface.size() * 4, cudaMemcpyHostToDevice, s));
-    CKD(cudaMemcpyAsync(dv.iface_info, pl.iface_info.data(), pl.iface_info.size() * 4, cudaMemcpyHostToDevice, s));
+  if (pl.v2) {
+    CKD(cudaMemcpyAsync((void *)pl.d2.units, pl.units2.data(), pl.units2.size() * sizeof(Bte2Unit), cudaMemcpyHostToDevice, s));
+  } else {
+    if (dv.n_iface) {
+      CKD(cudaMemcpyAsync(dv.iface, pl.iface.data(), pl.iface.size() * 4, cudaMemcpyHostToDevice, s));
+      CKD(cudaMemcpyAsync(dv.iface_info, pl.iface_info.data(), pl.iface_info.size() * 4, cudaMemcpyHostToDevice, s));
+    }
+    CKD(cudaMemcpyAsync((void *)dv.item_coef, pl.item_coef.data(), pl.item_coef.size() * 4, cudaMemcpyHostToDevice, s));
+    CKD(cudaMemcpyAsync(dv.units, pl.units.data(), pl.units.size() * sizeof(BteUnit), cudaMemcpyHostToDevice, s));
+    CKD(cudaMemcpyAsync(dv.band, pl.band.data(), pl.band.size() * 8, cudaMemcpyHostToDevice, s));
   }
-  CKD(cudaMemcpyAsync((void *)dv.item_coef, pl.item_coef.data(), pl.item_coef.size() * 4, cudaMemcpyHostToDevice, s));
-  CKD(cudaMemcpyAsync(dv.units, pl.units.data(), pl.units.size() * sizeof(BteUnit), cudaMemcpyHostToDevice, s));
-  CKD(cudaMemcpyAsync(dv.band, pl.band.data(), pl.band.size() * 8, cudaMemcpyHostToDevice, s));
   // coefficient table in the compute type
   if (dv.fp32) {
     h->coef_bytes.resize(pl.coef.size() * 4);
@@ -424,7 +583,8 @@ bte_status bte_create(const bte_problem *p, void *d_workspace, size_t bytes, voi
     h->coef_bytes.resize(pl.coef.size() * 8);
     std::memcpy(h->coef_bytes.data(), pl.coef.data(), pl.coef.size() * 8);
   }
-  st = dv.fp32 ? setup_sweep<float>(h) : setup_sweep<double>(h);
+  if (pl.v2) st = dv.fp32 ? setup_sweep2<float>(h) : setup_sweep2<double>(h);
+  else st = dv.fp32 ? setup_sweep<float>(h) : setup_sweep<double>(h);
   if (st != BTE_OK) return fail(st);
   st = skew(h, dv.Qphys, 0.0, 2, s);                       // cell codes -> skewed copies
   if (st == BTE_OK) st = skew(h, dv.Qphys, 1.0 / pl.sumC, 0, s);  // Q / sum C (Eq. 11)
@@ -442,6 +602,7 @@ bte_status bte_iterate(bte_solver *h, int32_t n, void *cuda_stream) {
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   h->last_stream = s;
   if (n == 0) return BTE_OK;
+  if (h->pl.v2) return h->pl.dev.fp32 ? iterate2_T<float>(h, n, h->pl.cf32, s) : iterate2_T<double>(h, n, h->pl.cf64, s);
   return h->pl.dev.fp32 ? iterate_T<float>(h, n, s) : iterate_T<double>(h, n, s);
 }
 
@@ -525,6 +686,10 @@ bte_status bte_solve_host(bte_solver *h, const double *Q_host, int32_t n, int32_
   if (reset) {
     CK(cudaMemsetAsync(h->ws + pl.state_begin, 0, pl.state_end - pl.state_begin, s));
     h->iters = 0;
+    if (pl.v2) {   // dT = 0 into the skewed class copies the sweep reads
+      bte_status st = skew(h, dv.dT, 1.0, 1, s);
+      if (st != BTE_OK) return st;
+    }
   }
   bte_status st = bte_iterate(h, n, cuda_stream);
   if (st != BTE_OK) return st;
@@ -544,11 +709,15 @@ int32_t bte_kernel_launches_per_iteration(const bte_solver *h) { return h ? h->l
 void bte_schedule_info(const bte_solver *h, int64_t out[6]) {
   if (!h || !out) return;
   const Plan &pl = h->pl;
-  out[0] = pl.dev.n_units;
+  out[0] = pl.v2 ? pl.d2.n_units : pl.dev.n_units;
   out[1] = h->sweep_grid;
   out[2] = pl.nthreads;
   out[3] = pl.steps_total;
   out[4] = pl.steps_total * pl.nthreads * BTE_P;
+  if (pl.v2) {
+    out[4] = 0;
+    for (const Bte2Unit &u : pl.units2) out[4] += (int64_t)pl.d2.nsteps * pl.d2.W * 32 * 4 * BTE2_P * u.nb;
+  }
   out[5] = (int64_t)pl.total;
 }
 

@@ -485,3 +485,5 @@ __global__ void bte_skew_kernel(const __grid_constant__ BteDev P, const double *
     if (which == 1) { P.dT[c] = solid ? src[c] : 0.0; }
   }
 }
+
+#include "bte_sweep2.cuh"

@@ -1,0 +1,602 @@
+// Fast path ("v2") of the B200 phonon-BTE sweep: 3-D, unmasked or masked-by-fallback, 16 directions per
+// octant, mirror-symmetric quadrature, <= 16 bands.  DESIGN.md "Kernels / sweep v2".
+//
+// Mapping.  One CTA = W warps sweeps one tile = 64 (y') x 2W (z') rows along x' for one octant and
+// one band group (NB = 1 or 2 bands x 16 directions).  Thread (J = lane, K = warp) owns the 2x2
+// row patch j' = 64 ty + 2J + {0,1}, k' = 2W tz + 2K + {0,1} and marches i' = t - J - K
+// (lane/warp-skewed wavefront), so that
+//   x-upwind  = its own register (carry),
+//   y-upwind  = its own patch row jj=0, or lane J-1's jj=1 row of the previous step (one SHFL),
+//   z-upwind  = its own patch row kk=0, or warp K-1's kk=1 row of the previous step (16-byte
+//               shared-memory exchange, double buffered),
+// i.e. 64 NB updates per thread and step need 32 NB shuffles and 16 NB 16-byte LDS/STS.  The
+// recurrence/moment coefficients are warp-uniform kernel parameters (constant bank -> uniform
+// registers), so an update is 8 FMA-pipe instructions with two vector-register operands each.
+// The (band x direction) intensity lives in registers only; tile faces go through L2-resident
+// planes (hand-off to the downstream tile, or the lagged boundary store at box faces).
+//
+// Scheduling.  Persistent CTAs take tickets in a topological unit order.  Dependencies between
+// tiles are tracked per STEP, not per tile: every unit publishes its step count (release store)
+// every BTE2_PUB steps, and the downstream tile in y / z (and the previous band group on the same
+// tile, which owns the moment accumulator before it) only has to stay 32 / W / 1 steps behind.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "bte_internal.h"
+
+#define BTE2_P 16         // directions per octant
+#define BTE2_MAXB 16      // bands in the parameter table
+#define BTE2_PUB 8        // progress is published every PUB steps
+#define BTE2_TYROWS 64    // tile rows along y' (32 lanes x 2)
+
+template <typename T> struct Bte2Coefs {   // kernel parameter (constant bank 0)
+  T k[BTE2_MAXB][BTE2_P][8];   // inv, ax, ay, az, w/tau, v w|sx|, v w|sy|, v w|sz|
+  T bc[BTE2_MAXB][2];          // C/4pi, C tau/(4pi sumC)
+};
+
+struct Bte2Unit {
+  int32_t oct, g, ty, tz;
+  int32_t dep_y, dep_z, dep_prev;   // unit ids (same octant) or -1
+  int32_t b0, nb;                   // first band, bands in this group (1 or 2)
+  int32_t pad[3];
+};
+
+struct Bte2Oct {
+  int32_t sx, sy, sz, cls;
+  void *M;                  // T [NS][4]   moment accumulator of this octant (skewed class layout)
+  void *xin, *xout;         // x face planes
+  void *ypl, *zpl;          // y / z face planes, slots 0..nty / 0..ntz
+};
+
+struct Bte2Dev {
+  int32_t nx, ny, nz, B;
+  int32_t W, nty, ntz, NU;          // warps per CTA; tiles along y', z'; nx + 31
+  int32_t nsteps, n_units, epoch, pad0;
+  int64_t NS;                       // nz * nty * NU * 64
+  void *dTQ[4];                     // T2 [NS]: (dT, Q / sum C) per x/y-flip class
+  Bte2Oct oct[8];
+  const Bte2Unit *units;
+  int32_t *prog;                    // [n_units] epoch << 16 | steps published
+  int32_t *ticket;
+  // boundary conditions (box faces x-,x+,y-,y+,z-,z+) and the update kernel
+  int32_t face_type[6];
+  double face_e0[6][BTE2_MAXB];     // isothermal inflow C_b dT_w / 4pi (Eq. 5)
+  double Pi_face[6];                // discrete hemispherical normaliser (reading G10)
+  double wsa[BTE2_P][3];            // w_p |s_p,a|
+  void *Gf;                         // T diffuse inflow [f][b][tb][ta]
+  int64_t gf_off[6];
+  double *dT, *q, *qmag, *red;      // fp64 outputs in physical layout; residual partials
+  int32_t n_red_blocks, pad1;
+  int64_t ncell;
+  double inv_sumCtau;
+};
+
+// ------------------------------------------------------------------ layouts (host + device)
+template <typename T> struct alignas(16) Bte2Chunk { T v[16 / sizeof(T)]; };   // 4 floats / 2 doubles
+template <typename T> struct alignas(2 * sizeof(T)) Bte2Pair { T x, y; };
+template <typename T> struct alignas(16) Bte2Mom { T v[4]; };
+
+#define BTE2_HD __host__ __device__ __forceinline__
+
+// skewed cell index: oriented i', j' of the class, physical k
+BTE2_HD int64_t sk2_index(int nty, int NU, int ip, int jp, int k) {
+  const int ty = jp >> 6, r = jp & 63, J = r >> 1, jj = r & 1;
+  return ((((int64_t)k * nty + ty) * NU + (ip + J)) * 2 + jj) * 32 + J;
+}
+// x planes: [tile][b][K][kk][jj][chunk][J], chunk = p / CP
+template <typename T>
+BTE2_HD int64_t xpl2_index(const Bte2Dev &P, int ty, int tz, int b, int K, int kk, int jj, int ch, int J) {
+  constexpr int NCH = BTE2_P * sizeof(T) / 16;
+  return ((((((int64_t)(tz * P.nty + ty) * P.B + b) * P.W + K) * 2 + kk) * 2 + jj) * NCH + ch) * 32 + J;
+}
+// y planes: [slot][tz][b][K][i'][kk][chunk]
+template <typename T>
+BTE2_HD int64_t ypl2_index(const Bte2Dev &P, int slot, int tz, int b, int K, int ip, int kk, int ch) {
+  constexpr int NCH = BTE2_P * sizeof(T) / 16;
+  return (((((int64_t)(slot * P.ntz + tz) * P.B + b) * P.W + K) * P.nx + ip) * 2 + kk) * NCH + ch;
+}
+// z planes: [slot][ty][b][u][jj][chunk][J], u = i' + J
+template <typename T>
+BTE2_HD int64_t zpl2_index(const Bte2Dev &P, int slot, int ty, int b, int u, int jj, int ch, int J) {
+  constexpr int NCH = BTE2_P * sizeof(T) / 16;
+  return (((((int64_t)(slot * P.nty + ty) * P.B + b) * P.NU + u) * 2 + jj) * NCH + ch) * 32 + J;
+}
+
+#ifdef __CUDACC__
+// ------------------------------------------------------------------ device helpers
+__device__ __forceinline__ int ld_acquire_gpu(const int *p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_gpu(int *p, int v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void *smem_dst, const void *gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  if (BYTES == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+  else if (BYTES == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+template <typename T> __device__ __forceinline__ Bte2Chunk<T> ldcg_chunk(const Bte2Chunk<T> *p) {
+  const float4 v = __ldcg(reinterpret_cast<const float4 *>(p));
+  Bte2Chunk<T> r;
+  memcpy(&r, &v, 16);
+  return r;
+}
+template <typename T> __device__ __forceinline__ T shfl_up1(T v);
+template <> __device__ __forceinline__ float shfl_up1<float>(float v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+template <> __device__ __forceinline__ double shfl_up1<double>(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+
+// shared-memory carve-up of one CTA
+template <typename T, int NB, int W> struct Bte2Smem {
+  static constexpr int CP = 16 / sizeof(T);            // directions per 16-byte chunk
+  static constexpr int NCH = BTE2_P / CP;              // chunks per band
+  static constexpr int NC = NB * NCH;                  // chunks per row and step
+  typedef Bte2Chunk<T> Ch;
+  Ch zbuf[2][W + 1][2][NC][32];      // [parity][slot: 0 = inflow plane, K+1 = written by warp K][jj][chunk][lane]
+  Ch ybuf[2][W][2][NC];              // [parity][warp][kk][chunk]: y inflow of lane 0
+  Bte2Mom<T> mold[2][2][W * 32];     // [kk][jj][tid] previous content of the moment accumulator
+  Bte2Pair<T> inp[2][2][2][W * 32];  // [parity][kk][jj][tid] (dT, Q/sumC) of the cell
+  int cache[4];                      // progress (steps) last seen of dep_y, dep_z, dep_prev
+};
+
+// ------------------------------------------------------------------ one unit = (octant, band group, tile)
+template <typename T, int NB, int W>
+__device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<T> &CF, const Bte2Unit &un,
+                                              unsigned char *smem_raw, int unit) {
+  typedef Bte2Smem<T, NB, W> SM;
+  SM *S = reinterpret_cast<SM *>(smem_raw);
+  constexpr int CP = SM::CP, NCH = SM::NCH, NC = SM::NC, NT = W * 32;
+  typedef Bte2Chunk<T> Ch;
+  const int tid = threadIdx.x, J = tid & 31, K = tid >> 5;
+  const Bte2Oct &O = P.oct[un.oct];
+  const int ty = un.ty, tz = un.tz, b0 = un.b0;
+  const int jp0 = ty * 64 + 2 * J, kp0 = tz * 2 * W + 2 * K;
+  const bool vk[2] = {kp0 < P.nz, kp0 + 1 < P.nz};
+  const bool vthread = (jp0 < P.ny) && vk[0];
+  const int jl = min(P.ny, (ty + 1) * 64) - 1 - ty * 64, kl = min(P.nz, (tz + 1) * 2 * W) - 1 - tz * 2 * W;
+  const int Jl = jl >> 1, jjl = jl & 1, Kl = kl >> 1, kkl = kl & 1;
+  const bool first = un.dep_prev < 0;                  // first band group of this octant: M is written, not added to
+  const int ebase = P.epoch << 16;
+
+  const Ch *xin = reinterpret_cast<const Ch *>(O.xin);
+  Ch *xout = reinterpret_cast<Ch *>(O.xout);
+  Ch *ypl = reinterpret_cast<Ch *>(O.ypl);
+  Ch *zpl = reinterpret_cast<Ch *>(O.zpl);
+  Bte2Mom<T> *M = reinterpret_cast<Bte2Mom<T> *>(O.M);
+  const Bte2Pair<T> *dTQ = reinterpret_cast<const Bte2Pair<T> *>(P.dTQ[O.cls]);
+
+  // cell index of row (jj,kk) at step t: base[kk] + jj*32 + (t - K) * 64
+  int64_t cbase[2];
+#pragma unroll
+  for (int kk = 0; kk < 2; ++kk) {
+    const int kp = kp0 + kk, k = vk[kk] ? (O.sz > 0 ? kp : P.nz - 1 - kp) : 0;
+    cbase[kk] = (((int64_t)k * P.nty + ty) * P.NU) * 64 + J;
+  }
+
+  // ---- progress of the units this one follows (uniform; smem cache + poll by threads 0..2)
+  auto wait_deps = [&](int t) {
+    const int need0 = t + 33, need1 = t + 1 + W, need2 = t + 1;
+    if (S->cache[0] < need0 || S->cache[1] < need1 || S->cache[2] < need2) {
+      __syncthreads();
+      if (tid < 3) {
+        const int dep = tid == 0 ? un.dep_y : (tid == 1 ? un.dep_z : un.dep_prev);
+        const int need = tid == 0 ? need0 : (tid == 1 ? need1 : need2);
+        int v;
+        while ((v = ld_acquire_gpu(P.prog + dep) - ebase) < need) __nanosleep(100);
+        S->cache[tid] = v;
+      }
+      __syncthreads();
+    }
+  };
+  if (tid < 3) {
+    const int dep = tid == 0 ? un.dep_y : (tid == 1 ? un.dep_z : un.dep_prev);
+    S->cache[tid] = dep < 0 ? 0x7fffffff : 0;
+  }
+  __syncthreads();
+  wait_deps(-1);
+
+  // ---- asynchronous prefetch (global -> shared) of everything step t1 consumes
+  auto prefetch = [&](int t1, int par) {
+    // (dT, Q) of the four cells
+    const int ip1 = t1 - J - K;
+    if (vthread && ip1 >= 0 && ip1 < P.nx) {
+#pragma unroll
+      for (int kk = 0; kk < 2; ++kk)
+        if (vk[kk]) {
+#pragma unroll
+          for (int jj = 0; jj < 2; ++jj)
+            cp_async<sizeof(Bte2Pair<T>)>(&S->inp[par][kk][jj][tid], dTQ + cbase[kk] + jj * 32 + (int64_t)(t1 - K) * 64);
+        }
+    }
+    // z inflow plane of warp 0 -> zbuf slot 0
+    if (t1 < P.NU) {
+#pragma unroll
+      for (int q = 0; q < (2 * NC * 32) / NT; ++q) {
+        const int e = tid + q * NT, b = e / (2 * NCH * 32), rem = e % (2 * NCH * 32);
+        const int jj = rem / (NCH * 32), ch = (rem / 32) % NCH, l = rem & 31;
+        cp_async<16>(&S->zbuf[par][0][jj][b * NCH + ch][l], zpl + zpl2_index<T>(P, tz, ty, b0 + b, t1, 0, 0, 0) + rem);
+      }
+    }
+    // y inflow of lane 0 of every warp -> ybuf
+    {
+      const int ipy = t1 - K;
+      if (J < 2 * NC && ipy >= 0 && ipy < P.nx) {
+        const int b = J / (2 * NCH), kk = (J / NCH) & 1, ch = J % NCH;
+        cp_async<16>(&S->ybuf[par][K][kk][b * NCH + ch], ypl + ypl2_index<T>(P, ty, tz, b0 + b, K, ipy, kk, ch));
+      }
+    }
+  };
+
+  // ---- x inflow -> carry registers (kept untouched by a thread until its first active step)
+  T c[2][2][NB * BTE2_P];                             // [jj][kk][b*16 + p]
+#pragma unroll
+  for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+    for (int jj = 0; jj < 2; ++jj)
+#pragma unroll
+      for (int b = 0; b < NB; ++b)
+#pragma unroll
+        for (int ch = 0; ch < NCH; ++ch) {
+          const Ch v = ldcg_chunk<T>(xin + xpl2_index<T>(P, ty, tz, b0 + b, K, kk, jj, ch, J));
+#pragma unroll
+          for (int q = 0; q < CP; ++q) c[jj][kk][b * BTE2_P + ch * CP + q] = v.v[q];
+        }
+
+  prefetch(0, 0);
+  cp_async_wait_all();
+  __syncthreads();
+
+  T bcx[NB], bcy[NB];
+#pragma unroll
+  for (int b = 0; b < NB; ++b) { bcx[b] = CF.bc[b0 + b][0]; bcy[b] = CF.bc[b0 + b][1]; }
+
+  for (int t = 0; t < P.nsteps; ++t) {
+    const int cur = t & 1, nxt = cur ^ 1;
+    const int ip = t - J - K;
+    const bool act = vthread && ip >= 0 && ip < P.nx;
+    wait_deps(t);
+    // previous content of the moment accumulator (this step) + everything step t+1 reads
+    if (act && !first) {
+#pragma unroll
+      for (int kk = 0; kk < 2; ++kk)
+        if (vk[kk]) {
+#pragma unroll
+          for (int jj = 0; jj < 2; ++jj) {
+            const Bte2Mom<T> *src = M + cbase[kk] + jj * 32 + (int64_t)(t - K) * 64;
+#pragma unroll
+            for (int h = 0; h < (int)sizeof(Bte2Mom<T>) / 16; ++h)
+              cp_async<16>(reinterpret_cast<char *>(&S->mold[kk][jj][tid]) + 16 * h, reinterpret_cast<const char *>(src) + 16 * h);
+          }
+        }
+    }
+    prefetch(t + 1, nxt);
+
+    T m[2][2][4];
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+      for (int b = 0; b < 2; ++b)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) m[a][b][q] = (T)0;
+
+    Bte2Pair<T> in[2][2];
+#pragma unroll
+    for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+      for (int jj = 0; jj < 2; ++jj) in[jj][kk] = S->inp[cur][kk][jj][tid];
+
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+      T r[2][2];
+#pragma unroll
+      for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+        for (int jj = 0; jj < 2; ++jj) r[jj][kk] = fma(bcx[b], in[jj][kk].x, bcy[b] * in[jj][kk].y);
+#pragma unroll
+      for (int ch = 0; ch < NCH; ++ch) {
+        const int q0 = b * BTE2_P + ch * CP, cn = b * NCH + ch;
+        // y inflow: lane J-1's jj=1 rows of the previous step; lane 0: the staged plane
+        T yin[2][CP];
+#pragma unroll
+        for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+          for (int q = 0; q < CP; ++q) yin[kk][q] = shfl_up1<T>(c[1][kk][q0 + q]);
+        if (J == 0) {
+#pragma unroll
+          for (int kk = 0; kk < 2; ++kk) {
+            const Ch v = S->ybuf[cur][K][kk][cn];
+#pragma unroll
+            for (int q = 0; q < CP; ++q) yin[kk][q] = v.v[q];
+          }
+        }
+        // z inflow: slot K (warp K-1's kk=1 rows of the previous step, or the staged plane)
+        const Ch z0 = S->zbuf[cur][K][0][cn][J], z1 = S->zbuf[cur][K][1][cn][J];
+        if (act) {
+          Ch o0, o1;
+#pragma unroll
+          for (int q = 0; q < CP; ++q) {
+            const int p = ch * CP + q;
+            const T inv = CF.k[b0 + b][p][0], ax = CF.k[b0 + b][p][1], ay = CF.k[b0 + b][p][2], az = CF.k[b0 + b][p][3];
+            const T w0 = CF.k[b0 + b][p][4], w1 = CF.k[b0 + b][p][5], w2 = CF.k[b0 + b][p][6], w3 = CF.k[b0 + b][p][7];
+            T e00 = r[0][0] * inv; e00 = fma(ax, c[0][0][q0 + q], e00); e00 = fma(ay, yin[0][q], e00); e00 = fma(az, z0.v[q], e00);
+            T e10 = r[1][0] * inv; e10 = fma(ax, c[1][0][q0 + q], e10); e10 = fma(az, z1.v[q], e10); e10 = fma(ay, e00, e10);
+            T e01 = r[0][1] * inv; e01 = fma(ax, c[0][1][q0 + q], e01); e01 = fma(ay, yin[1][q], e01); e01 = fma(az, e00, e01);
+            T e11 = r[1][1] * inv; e11 = fma(ax, c[1][1][q0 + q], e11); e11 = fma(ay, e01, e11); e11 = fma(az, e10, e11);
+            c[0][0][q0 + q] = e00; c[1][0][q0 + q] = e10; c[0][1][q0 + q] = e01; c[1][1][q0 + q] = e11;
+            o0.v[q] = e01; o1.v[q] = e11;
+            m[0][0][0] = fma(w0, e00, m[0][0][0]); m[0][0][1] = fma(w1, e00, m[0][0][1]); m[0][0][2] = fma(w2, e00, m[0][0][2]); m[0][0][3] = fma(w3, e00, m[0][0][3]);
+            m[1][0][0] = fma(w0, e10, m[1][0][0]); m[1][0][1] = fma(w1, e10, m[1][0][1]); m[1][0][2] = fma(w2, e10, m[1][0][2]); m[1][0][3] = fma(w3, e10, m[1][0][3]);
+            m[0][1][0] = fma(w0, e01, m[0][1][0]); m[0][1][1] = fma(w1, e01, m[0][1][1]); m[0][1][2] = fma(w2, e01, m[0][1][2]); m[0][1][3] = fma(w3, e01, m[0][1][3]);
+            m[1][1][0] = fma(w0, e11, m[1][1][0]); m[1][1][1] = fma(w1, e11, m[1][1][1]); m[1][1][2] = fma(w2, e11, m[1][1][2]); m[1][1][3] = fma(w3, e11, m[1][1][3]);
+          }
+          S->zbuf[nxt][K + 1][0][cn][J] = o0;
+          S->zbuf[nxt][K + 1][1][cn][J] = o1;
+        }
+      }
+    }
+
+    cp_async_wait_all();                 // mold of this step and the planes / inputs of the next one have landed
+    if (act) {
+      // (b) moments of this band group into the octant accumulator (one owner per cell and group)
+#pragma unroll
+      for (int kk = 0; kk < 2; ++kk)
+        if (vk[kk]) {
+#pragma unroll
+          for (int jj = 0; jj < 2; ++jj) {
+            Bte2Mom<T> o;
+            if (first) {
+#pragma unroll
+              for (int q = 0; q < 4; ++q) o.v[q] = m[jj][kk][q];
+            } else {
+              const Bte2Mom<T> old = S->mold[kk][jj][tid];
+#pragma unroll
+              for (int q = 0; q < 4; ++q) o.v[q] = old.v[q] + m[jj][kk][q];
+            }
+            M[cbase[kk] + jj * 32 + (int64_t)(t - K) * 64] = o;
+          }
+        }
+      // outflow faces: tile hand-off / lagged boundary store
+      if (J == Jl) {
+#pragma unroll
+        for (int b = 0; b < NB; ++b)
+#pragma unroll
+          for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+            for (int ch = 0; ch < NCH; ++ch) {
+              Ch o;
+#pragma unroll
+              for (int q = 0; q < CP; ++q) o.v[q] = jjl ? c[1][kk][b * BTE2_P + ch * CP + q] : c[0][kk][b * BTE2_P + ch * CP + q];
+              ypl[ypl2_index<T>(P, ty + 1, tz, b0 + b, K, ip, kk, ch)] = o;
+            }
+      }
+      if (K == Kl) {
+#pragma unroll
+        for (int b = 0; b < NB; ++b)
+#pragma unroll
+          for (int jj = 0; jj < 2; ++jj)
+#pragma unroll
+            for (int ch = 0; ch < NCH; ++ch) {
+              Ch o;
+#pragma unroll
+              for (int q = 0; q < CP; ++q) o.v[q] = kkl ? c[jj][1][b * BTE2_P + ch * CP + q] : c[jj][0][b * BTE2_P + ch * CP + q];
+              zpl[zpl2_index<T>(P, tz + 1, ty, b0 + b, t - K, jj, ch, J)] = o;
+            }
+      }
+    }
+    __syncthreads();
+    if ((t & (BTE2_PUB - 1)) == BTE2_PUB - 1 && tid == 0) {
+      __threadfence();
+      st_release_gpu(P.prog + unit, ebase + t + 1);
+    }
+  }
+
+  // ---- x outflow (carries are final: a thread stops updating them after its last active step)
+#pragma unroll
+  for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+    for (int jj = 0; jj < 2; ++jj)
+#pragma unroll
+      for (int b = 0; b < NB; ++b)
+#pragma unroll
+        for (int ch = 0; ch < NCH; ++ch) {
+          Ch o;
+#pragma unroll
+          for (int q = 0; q < CP; ++q) o.v[q] = c[jj][kk][b * BTE2_P + ch * CP + q];
+          xout[xpl2_index<T>(P, ty, tz, b0 + b, K, kk, jj, ch, J)] = o;
+        }
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) st_release_gpu(P.prog + unit, ebase + 0xffff);
+}
+
+template <typename T, int W>
+__global__ void __launch_bounds__(W * 32) bte2_sweep_kernel(const __grid_constant__ Bte2Dev P,
+                                                            const __grid_constant__ Bte2Coefs<T> CF) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int NBMAX = sizeof(T) == 4 ? 2 : 1;
+  __shared__ int s_unit;
+  for (;;) {
+    __syncthreads();
+    if (threadIdx.x == 0) s_unit = atomicAdd(P.ticket, 1);
+    __syncthreads();
+    const int unit = s_unit;
+    if (unit >= P.n_units) break;
+    const Bte2Unit un = P.units[unit];
+    if (NBMAX == 2 && un.nb == 2) bte2_run_unit<T, NBMAX, W>(P, CF, un, smem_raw, unit);
+    else bte2_run_unit<T, 1, W>(P, CF, un, smem_raw, unit);
+  }
+}
+
+// ------------------------------------------------------------------ boundary kernels (v2 layouts)
+// chunk holding direction p of band b on the face plane of octant o, axis a, at oriented cell (ip,jp,kp);
+// side 0 = inflow plane, 1 = outflow plane
+template <typename T>
+__device__ __forceinline__ Bte2Chunk<T> *bte2_plane_chunk(const Bte2Dev &P, int o, int a, int side, int b, int ch,
+                                                          int ip, int jp, int kp) {
+  const Bte2Oct &O = P.oct[o];
+  if (a == 0) {
+    const int ty = jp >> 6, J = (jp & 63) >> 1, jj = jp & 1, tz = kp / (2 * P.W), K = (kp % (2 * P.W)) >> 1, kk = kp & 1;
+    return reinterpret_cast<Bte2Chunk<T> *>(side ? O.xout : O.xin) + xpl2_index<T>(P, ty, tz, b, K, kk, jj, ch, J);
+  }
+  if (a == 1) {
+    const int tz = kp / (2 * P.W), K = (kp % (2 * P.W)) >> 1, kk = kp & 1;
+    return reinterpret_cast<Bte2Chunk<T> *>(O.ypl) + ypl2_index<T>(P, side ? P.nty : 0, tz, b, K, ip, kk, ch);
+  }
+  const int ty = jp >> 6, J = (jp & 63) >> 1, jj = jp & 1;
+  return reinterpret_cast<Bte2Chunk<T> *>(O.zpl) + zpl2_index<T>(P, side ? P.ntz : 0, ty, b, ip + J, jj, ch, J);
+}
+
+struct Bte2Face { int na, nb; };
+__device__ __forceinline__ Bte2Face bte2_face(const Bte2Dev &P, int a) {
+  Bte2Face g;
+  if (a == 0) { g.na = P.ny; g.nb = P.nz; } else if (a == 1) { g.na = P.nx; g.nb = P.nz; } else { g.na = P.nx; g.nb = P.ny; }
+  return g;
+}
+// oriented coordinates of the boundary cell (ta, tb) of face axis a for octant o
+__device__ __forceinline__ void bte2_face_cell(const Bte2Dev &P, int o, int a, int side_phys, int ta, int tb, int &ip, int &jp, int &kp) {
+  const Bte2Oct &O = P.oct[o];
+  int i, j, k;
+  if (a == 0) { i = side_phys ? P.nx - 1 : 0; j = ta; k = tb; }
+  else if (a == 1) { j = side_phys ? P.ny - 1 : 0; i = ta; k = tb; }
+  else { k = side_phys ? P.nz - 1 : 0; i = ta; j = tb; }
+  ip = O.sx > 0 ? i : P.nx - 1 - i; jp = O.sy > 0 ? j : P.ny - 1 - j; kp = O.sz > 0 ? k : P.nz - 1 - k;
+}
+
+// G_{f,b}(cell) = (1/Pi_f) sum_{s.n>0} w (s.n) e^n for DIFFUSE box faces (Eq. 6, reading G10)
+template <typename T>
+__global__ void bte2_gdiff_kernel(const __grid_constant__ Bte2Dev P) {
+  constexpr int CP = 16 / sizeof(T), NCH = BTE2_P / CP;
+  T *Gf = reinterpret_cast<T *>(P.Gf);
+  for (int f = 0; f < 6; ++f) {
+    if (P.face_type[f] != 1) continue;
+    const int a = f >> 1, side = f & 1;
+    const Bte2Face g = bte2_face(P, a);
+    const int64_t nf = (int64_t)g.na * g.nb * P.B;
+    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < nf; e += (int64_t)gridDim.x * blockDim.x) {
+      const int ta = (int)(e % g.na), tb = (int)((e / g.na) % g.nb), b = (int)(e / ((int64_t)g.na * g.nb));
+      double H = 0.0;
+      for (int o = 0; o < 8; ++o) {
+        const Bte2Oct &O = P.oct[o];
+        const int sg = a == 0 ? O.sx : (a == 1 ? O.sy : O.sz);
+        if ((sg > 0) != (side == 1)) continue;          // outgoing octants only
+        int ip, jp, kp;
+        bte2_face_cell(P, o, a, side, ta, tb, ip, jp, kp);
+        for (int ch = 0; ch < NCH; ++ch) {
+          const Bte2Chunk<T> v = ldcg_chunk<T>(bte2_plane_chunk<T>(P, o, a, 1, b, ch, ip, jp, kp));
+#pragma unroll
+          for (int q = 0; q < CP; ++q) H += P.wsa[ch * CP + q][a] * (double)v.v[q];
+        }
+      }
+      Gf[P.gf_off[f] + e] = (T)(H / P.Pi_face[f]);
+    }
+  }
+}
+
+// Fill the inflow plane of every octant on every axis from the lagged outflow (Eq. 5-7 + periodic).
+template <typename T>
+__global__ void bte2_ghost_kernel(const __grid_constant__ Bte2Dev P) {
+  constexpr int CP = 16 / sizeof(T), NCH = BTE2_P / CP;
+  const T *Gf = reinterpret_cast<const T *>(P.Gf);
+  const int64_t gtid = blockIdx.x * (int64_t)blockDim.x + threadIdx.x, gstride = (int64_t)gridDim.x * blockDim.x;
+  for (int o = 0; o < 8; ++o) {
+    const Bte2Oct &O = P.oct[o];
+    for (int a = 0; a < 3; ++a) {
+      const int sg = a == 0 ? O.sx : (a == 1 ? O.sy : O.sz);
+      const int side = sg > 0 ? 0 : 1, f = 2 * a + side;   // physical face the octant enters through
+      const int type = P.face_type[f];
+      const Bte2Face g = bte2_face(P, a);
+      const int64_t n = (int64_t)g.na * g.nb * P.B * NCH;
+      for (int64_t e = gtid; e < n; e += gstride) {
+        // ta fastest, then chunk, so that neighbouring threads touch neighbouring lanes of a plane
+        const int ta = (int)(e % g.na), ch = (int)((e / g.na) % NCH), tb = (int)((e / ((int64_t)g.na * NCH)) % g.nb);
+        const int b = (int)(e / ((int64_t)g.na * NCH * g.nb));
+        int ip, jp, kp;
+        bte2_face_cell(P, o, a, side, ta, tb, ip, jp, kp);
+        Bte2Chunk<T> v;
+        if (type == 0) {
+#pragma unroll
+          for (int q = 0; q < CP; ++q) v.v[q] = (T)P.face_e0[f][b];
+        } else if (type == 1) {
+          const T gv = Gf[P.gf_off[f] + ((int64_t)b * g.nb + tb) * g.na + ta];
+#pragma unroll
+          for (int q = 0; q < CP; ++q) v.v[q] = gv;
+        } else if (type == 2) {   // specular: mirrored octant leaves through this face at the same cell
+          int ip2, jp2, kp2;
+          bte2_face_cell(P, o ^ (1 << a), a, side, ta, tb, ip2, jp2, kp2);
+          v = ldcg_chunk<T>(bte2_plane_chunk<T>(P, o ^ (1 << a), a, 1, b, ch, ip2, jp2, kp2));
+        } else {                  // periodic: same octant leaves through the opposite face
+          int ip2, jp2, kp2;
+          bte2_face_cell(P, o, a, side ^ 1, ta, tb, ip2, jp2, kp2);
+          v = ldcg_chunk<T>(bte2_plane_chunk<T>(P, o, a, 1, b, ch, ip2, jp2, kp2));
+        }
+        *bte2_plane_chunk<T>(P, o, a, 0, b, ch, ip, jp, kp) = v;
+      }
+    }
+  }
+  if (gtid == 0) *P.ticket = 0;
+}
+
+// ------------------------------------------------------------------ (c) update + residual, v2 layouts
+// dT^{n+1} = M0 / sum(C/tau) (Eq. 16), q = M1 (Eq. 4), residual partial sums (Eq. 23); octant partials are
+// summed in fp64 in a fixed order; dT is written back into the four skewed class copies the sweep reads.
+template <typename T>
+__global__ void __launch_bounds__(256) bte2_update_kernel(const __grid_constant__ Bte2Dev P) {
+  double sT = 0, mT = 0, sq = 0, mq = 0;
+  for (int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; c < P.ncell; c += (int64_t)gridDim.x * blockDim.x) {
+    const int i = (int)(c % P.nx), j = (int)((c / P.nx) % P.ny), k = (int)(c / ((int64_t)P.nx * P.ny));
+    int64_t sk[4];
+#pragma unroll
+    for (int cl = 0; cl < 4; ++cl)
+      sk[cl] = sk2_index(P.nty, P.NU, (cl & 1) ? P.nx - 1 - i : i, (cl & 2) ? P.ny - 1 - j : j, k);
+    double m0 = 0, m1 = 0, m2 = 0, m3 = 0;
+#pragma unroll
+    for (int o = 0; o < 8; ++o) {
+      const Bte2Oct &O = P.oct[o];
+      const Bte2Mom<T> *Mp = reinterpret_cast<const Bte2Mom<T> *>(O.M) + sk[o & 3];
+      T v[4];
+      if (sizeof(T) == 4) {
+        const float4 x = __ldcg(reinterpret_cast<const float4 *>(Mp));
+        memcpy(v, &x, 16);
+      } else {
+        const double2 x = __ldcg(reinterpret_cast<const double2 *>(Mp)), y = __ldcg(reinterpret_cast<const double2 *>(Mp) + 1);
+        memcpy(v, &x, 16); memcpy(reinterpret_cast<char *>(v) + 16, &y, 16);
+      }
+      m0 += (double)v[0]; m1 += O.sx * (double)v[1]; m2 += O.sy * (double)v[2]; m3 += O.sz * (double)v[3];
+    }
+    const double Tn = m0 * P.inv_sumCtau;
+    const double dlt = Tn - P.dT[c];
+    sT += dlt * dlt; mT = fmax(mT, fabs(Tn));
+    P.dT[c] = Tn;
+    P.q[c] = m1; P.q[P.ncell + c] = m2; P.q[2 * P.ncell + c] = m3;
+    const double qm = sqrt(m1 * m1 + m2 * m2 + m3 * m3);
+    const double dq = qm - P.qmag[c];
+    sq += dq * dq; mq = fmax(mq, qm);
+    P.qmag[c] = qm;
+#pragma unroll
+    for (int cl = 0; cl < 4; ++cl) reinterpret_cast<Bte2Pair<T> *>(P.dTQ[cl])[sk[cl]].x = (T)Tn;
+  }
+  block_reduce4(sT, mT, sq, mq);
+  if (threadIdx.x == 0) {
+    P.red[blockIdx.x] = sT; P.red[P.n_red_blocks + blockIdx.x] = mT;
+    P.red[2 * P.n_red_blocks + blockIdx.x] = sq; P.red[3 * P.n_red_blocks + blockIdx.x] = mq;
+  }
+}
+
+// physical fp64 field -> the four skewed class copies: which = 0: Q * scale -> .y ; 1: dT -> .x (and P.dT)
+template <typename T>
+__global__ void bte2_skew_kernel(const __grid_constant__ Bte2Dev P, const double *src, double scale, int which) {
+  for (int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; c < P.ncell; c += (int64_t)gridDim.x * blockDim.x) {
+    const int i = (int)(c % P.nx), j = (int)((c / P.nx) % P.ny), k = (int)(c / ((int64_t)P.nx * P.ny));
+    for (int cl = 0; cl < 4; ++cl) {
+      Bte2Pair<T> *d = reinterpret_cast<Bte2Pair<T> *>(P.dTQ[cl]) +
+                       sk2_index(P.nty, P.NU, (cl & 1) ? P.nx - 1 - i : i, (cl & 2) ? P.ny - 1 - j : j, k);
+      if (which == 0) d->y = (T)(src[c] * scale); else d->x = (T)src[c];
+    }
+    if (which == 1) P.dT[c] = src[c];
+  }
+}
+#endif  // __CUDACC__
