@@ -283,8 +283,11 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
   if (const char *e = std::getenv("BTE_FORCE_GENERIC")) if (e[0] == '1') v2 = false;
   for (int o = 0; o < 8 && v2; ++o) {
     if ((int)od[o].size() != BTE2_P) v2 = false;
-    for (int b = 0; b < B && v2; ++b)
-      if (pl.item_coef[(size_t)o * max_items + b] != pl.item_coef[b]) v2 = false;
+    for (int b = 0; b < B && v2; ++b) {   // same table up to rounding of the mirrored direction cosines
+      const double *x = pl.coef.data() + pl.item_coef[(size_t)o * max_items + b], *y = pl.coef.data() + pl.item_coef[b];
+      for (int c = 0; c < BTE_P * BTE_NCOEF && v2; ++c)
+        if (std::fabs(x[c] - y[c]) > 1e-12 * std::max(std::fabs(y[c]), 1e-300)) v2 = false;
+    }
   }
   pl.v2 = v2;
   if (v2) {

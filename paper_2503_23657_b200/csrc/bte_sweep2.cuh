@@ -185,9 +185,11 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
       if (tid < 3) {
         const int dep = tid == 0 ? un.dep_y : (tid == 1 ? un.dep_z : un.dep_prev);
         const int need = tid == 0 ? need0 : (tid == 1 ? need1 : need2);
-        int v;
-        while ((v = ld_acquire_gpu(P.prog + dep) - ebase) < need) __nanosleep(100);
-        S->cache[tid] = v;
+        if (dep >= 0) {
+          int v;
+          while ((v = ld_acquire_gpu(P.prog + dep) - ebase) < need) __nanosleep(100);
+          S->cache[tid] = v;
+        }
       }
       __syncthreads();
     }
