@@ -10,6 +10,7 @@
 #include <limits>
 #include <map>
 #include <new>
+#include <queue>
 #include <string>
 #include <vector>
 
@@ -279,7 +280,7 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
 
   // ---- fast path: 3-D, all solid, 16 directions in each of the 8 octants with identical |s|, w tables
   // (mirror-symmetric quadrature), <= 16 bands.  Anything else runs the generic kernels above.
-  bool v2 = p->dim == 3 && nif == 0 && nsolid == N && B <= BTE2_MAXB && p->nx <= 60000;
+  bool v2 = p->dim == 3 && nif == 0 && nsolid == N && B <= BTE2_MAXB && p->nx <= 60000 && p->ny % 2 == 0 && p->nz % 2 == 0;
   if (const char *e = std::getenv("BTE_FORCE_GENERIC")) if (e[0] == '1') v2 = false;
   for (int o = 0; o < 8 && v2; ++o) {
     if ((int)od[o].size() != BTE2_P) v2 = false;
@@ -292,11 +293,12 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
   pl.v2 = v2;
   if (v2) {
     Bte2Dev &d = pl.d2;
-    int W = p->nz >= 48 ? 8 : 4;
-    if (const char *e = std::getenv("BTE_V2_W")) { const int w = std::atoi(e); if (w == 4 || w == 8) W = w; }
+    int W = (p->nz >= 48 && dv.fp32) ? 8 : 4;   // fp64 staging buffers of 8 warps do not fit shared memory
+    if (const char *e = std::getenv("BTE_V2_W")) { const int w = std::atoi(e); if (w == 4 || (w == 8 && dv.fp32)) W = w; }
     d.nx = p->nx; d.ny = p->ny; d.nz = p->nz; d.B = B; d.W = W;
     d.nty = (p->ny + 63) / 64; d.ntz = (p->nz + 2 * W - 1) / (2 * W); d.NU = p->nx + 31;
     d.nsteps = p->nx + 31 + W - 1;
+    if (const char *e = std::getenv("BTE_V2_DBG")) d.dbg = std::atoi(e);
     d.NS = (int64_t)p->nz * d.nty * d.NU * 64;
     d.ncell = N; d.inv_sumCtau = dv.inv_sumCtau;
     const int NBmax = dv.fp32 ? 2 : 1, G = (B + NBmax - 1) / NBmax;
@@ -412,6 +414,56 @@ size_t bind(Plan &pl, unsigned char *ws) {
   return off;
 }
 
+// Ticket order of the fast path = start order of a list schedule simulated on `slots` resident CTAs:
+// a unit may start once every unit it follows is lag + BTE2_SLACK steps ahead, so that the per-step
+// dependency polls of the kernel (which stay in place for correctness) almost never have to wait.
+void order_units2(Plan &pl, int slots) {
+  std::vector<Bte2Unit> &U = pl.units2;
+  const int n = (int)U.size(), W = pl.d2.W, nsteps = pl.d2.nsteps;
+  const int NBmax = pl.dev.fp32 ? 2 : 1;
+  std::vector<double> start(n, -1.0), steptime(n);
+  std::vector<int> ndep(n, 0), order;
+  std::vector<std::vector<int>> succ(n);
+  for (int u = 0; u < n; ++u) {
+    steptime[u] = (double)U[u].nb / NBmax;
+    const int deps[3] = {U[u].dep_y, U[u].dep_z, U[u].dep_prev};
+    for (int d : deps) if (d >= 0) { ++ndep[u]; succ[d].push_back(u); }
+  }
+  auto allowed = [&](int u) {
+    const int deps[3] = {U[u].dep_y, U[u].dep_z, U[u].dep_prev};
+    const int lag[3] = {33, W + 1, 1};
+    double a = 0;
+    for (int k = 0; k < 3; ++k)
+      if (deps[k] >= 0) a = std::max(a, start[deps[k]] + (lag[k] + BTE2_DIST + BTE2_SLACK + BTE2_PUB) * steptime[deps[k]]);
+    return a;
+  };
+  typedef std::pair<double, int> Key;
+  std::priority_queue<Key, std::vector<Key>, std::greater<Key>> ready, freeslot;
+  for (int u = 0; u < n; ++u) if (ndep[u] == 0) ready.push({0.0, u});
+  for (int k = 0; k < std::max(slots, 1); ++k) freeslot.push({0.0, k});
+  order.reserve(n);
+  while (!ready.empty()) {
+    const Key f = freeslot.top(); freeslot.pop();
+    const Key r = ready.top(); ready.pop();
+    const int u = r.second;
+    start[u] = std::max(f.first, r.first);
+    freeslot.push({start[u] + nsteps * steptime[u], f.second});
+    order.push_back(u);
+    for (int v : succ[u]) if (--ndep[v] == 0) ready.push({allowed(v), v});
+  }
+  std::vector<int> newid(n);
+  for (int k = 0; k < n; ++k) newid[order[k]] = k;
+  std::vector<Bte2Unit> out(n);
+  for (int k = 0; k < n; ++k) {
+    Bte2Unit x = U[order[k]];
+    if (x.dep_y >= 0) x.dep_y = newid[x.dep_y];
+    if (x.dep_z >= 0) x.dep_z = newid[x.dep_z];
+    if (x.dep_prev >= 0) x.dep_prev = newid[x.dep_prev];
+    out[k] = x;
+  }
+  U.swap(out);
+}
+
 }  // namespace
 
 struct bte_solver {
@@ -487,7 +539,7 @@ bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t
 template <typename T, int W>
 bte_status setup_sweep2_W(bte_solver *h) {
   Plan &pl = h->pl;
-  pl.smem2 = sizeof(Bte2Smem<T, sizeof(T) == 4 ? 2 : 1, W>);
+  pl.smem2 = sizeof(Bte2Smem<T, sizeof(T) == 4 ? 2 : 1, W, BTE2_DIST>);
   CK(cudaFuncSetAttribute(bte2_sweep_kernel<T, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem2));
   int occ = 0;
   CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bte2_sweep_kernel<T, W>, W * 32, pl.smem2));
@@ -563,9 +615,13 @@ bte_status bte_create(const bte_problem *p, void *d_workspace, size_t bytes, voi
   CKD(cudaGetDevice(&devid));
   CKD(cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, devid));
   CKD(cudaMemsetAsync(h->ws, 0, need, s));
+  if (pl.v2) st = dv.fp32 ? setup_sweep2<float>(h) : setup_sweep2<double>(h);
+  else st = dv.fp32 ? setup_sweep<float>(h) : setup_sweep<double>(h);
+  if (st != BTE_OK) return fail(st);
   CKD(cudaMemcpyAsync(dv.code, pl.code.data(), pl.code.size(), cudaMemcpyHostToDevice, s));
   CKD(cudaMemcpyAsync(dv.Qphys, pl.Q.data(), pl.Q.size() * 8, cudaMemcpyHostToDevice, s));
   if (pl.v2) {
+    order_units2(pl, h->sweep_grid);
     CKD(cudaMemcpyAsync((void *)pl.d2.units, pl.units2.data(), pl.units2.size() * sizeof(Bte2Unit), cudaMemcpyHostToDevice, s));
   } else {
     if (dv.n_iface) {
@@ -586,9 +642,7 @@ bte_status bte_create(const bte_problem *p, void *d_workspace, size_t bytes, voi
     h->coef_bytes.resize(pl.coef.size() * 8);
     std::memcpy(h->coef_bytes.data(), pl.coef.data(), pl.coef.size() * 8);
   }
-  if (pl.v2) st = dv.fp32 ? setup_sweep2<float>(h) : setup_sweep2<double>(h);
-  else st = dv.fp32 ? setup_sweep<float>(h) : setup_sweep<double>(h);
-  if (st != BTE_OK) return fail(st);
+
   st = skew(h, dv.Qphys, 0.0, 2, s);                       // cell codes -> skewed copies
   if (st == BTE_OK) st = skew(h, dv.Qphys, 1.0 / pl.sumC, 0, s);  // Q / sum C (Eq. 11)
   if (st != BTE_OK) return fail(st);

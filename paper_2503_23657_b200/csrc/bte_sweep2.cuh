@@ -22,14 +22,18 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <type_traits>
+
 #include "bte_internal.h"
 
 #define BTE2_P 16         // directions per octant
 #define BTE2_MAXB 16      // bands in the parameter table
 #define BTE2_PUB 8        // progress is published every PUB steps
+#define BTE2_DIST 2       // cp.async prefetch distance in steps
+#define BTE2_SLACK 24     // extra steps a unit lets the units it follows get ahead before it starts
 #define BTE2_TYROWS 64    // tile rows along y' (32 lanes x 2)
 
-template <typename T> struct Bte2Coefs {   // kernel parameter (constant bank 0)
+template <typename T> struct alignas(16) Bte2Coefs {   // kernel parameter (constant bank 0)
   T k[BTE2_MAXB][BTE2_P][8];   // inv, ax, ay, az, w/tau, v w|sx|, v w|sy|, v w|sz|
   T bc[BTE2_MAXB][2];          // C/4pi, C tau/(4pi sumC)
 };
@@ -51,7 +55,7 @@ struct Bte2Oct {
 struct Bte2Dev {
   int32_t nx, ny, nz, B;
   int32_t W, nty, ntz, NU;          // warps per CTA; tiles along y', z'; nx + 31
-  int32_t nsteps, n_units, epoch, pad0;
+  int32_t nsteps, n_units, epoch, dbg;   // dbg: timing experiments only (BTE_V2_DBG), 0 in production
   int64_t NS;                       // nz * nty * NU * 64
   void *dTQ[4];                     // T2 [NS]: (dT, Q / sum C) per x/y-flip class
   Bte2Oct oct[8];
@@ -118,7 +122,8 @@ __device__ __forceinline__ void cp_async(void *smem_dst, const void *gsrc) {
   if (BYTES == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
   else if (BYTES == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
 }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 template <typename T> __device__ __forceinline__ Bte2Chunk<T> ldcg_chunk(const Bte2Chunk<T> *p) {
   const float4 v = __ldcg(reinterpret_cast<const float4 *>(p));
@@ -130,106 +135,132 @@ template <typename T> __device__ __forceinline__ T shfl_up1(T v);
 template <> __device__ __forceinline__ float shfl_up1<float>(float v) { return __shfl_up_sync(0xffffffffu, v, 1); }
 template <> __device__ __forceinline__ double shfl_up1<double>(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
 
-// shared-memory carve-up of one CTA
-template <typename T, int NB, int W> struct Bte2Smem {
+// shared-memory carve-up of one CTA.  D = prefetch distance in steps (ring of D+1 buffers).
+template <typename T, int NB, int W, int D> struct Bte2Smem {
   static constexpr int CP = 16 / sizeof(T);            // directions per 16-byte chunk
   static constexpr int NCH = BTE2_P / CP;              // chunks per band
   static constexpr int NC = NB * NCH;                  // chunks per row and step
   typedef Bte2Chunk<T> Ch;
-  Ch zbuf[2][W + 1][2][NC][32];      // [parity][slot: 0 = inflow plane, K+1 = written by warp K][jj][chunk][lane]
-  Ch ybuf[2][W][2][NC];              // [parity][warp][kk][chunk]: y inflow of lane 0
-  Bte2Mom<T> mold[2][2][W * 32];     // [kk][jj][tid] previous content of the moment accumulator
-  Bte2Pair<T> inp[2][2][2][W * 32];  // [parity][kk][jj][tid] (dT, Q/sumC) of the cell
-  int cache[4];                      // progress (steps) last seen of dep_y, dep_z, dep_prev
+  Ch zex[2][W][2][NC][32];           // [parity][K][jj][chunk][lane]: kk=1 rows of warp K, read by warp K+1 / copied out
+  Ch zin0[D + 1][2][NC][32];         // staged z inflow plane of warp 0
+  Ch ybuf[D + 1][W][2][NC];          // [ring][warp][kk][chunk]: y inflow of lane 0
+  Ch yst[2][W][2 * NC];              // [parity][warp][kk*NC + chunk]: jj=1 rows of lane Jl, copied out one step later
+  Bte2Mom<T> mold[2][2][2][W * 32];  // [parity][kk][jj][tid] previous content of the moment accumulator
+  Bte2Pair<T> inp[D + 1][2][2][W * 32];    // [ring][kk][jj][tid] (dT, Q/sumC) of the cell
 };
 
 // ------------------------------------------------------------------ one unit = (octant, band group, tile)
-template <typename T, int NB, int W>
+template <typename T, int NB, int W, int D>
 __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<T> &CF, const Bte2Unit &un,
                                               unsigned char *smem_raw, int unit) {
-  typedef Bte2Smem<T, NB, W> SM;
+  typedef Bte2Smem<T, NB, W, D> SM;
   SM *S = reinterpret_cast<SM *>(smem_raw);
-  constexpr int CP = SM::CP, NCH = SM::NCH, NC = SM::NC, NT = W * 32;
+  constexpr int CP = SM::CP, NCH = SM::NCH, NC = SM::NC, NT = W * 32, R = D + 1;
   typedef Bte2Chunk<T> Ch;
+  const unsigned FULL = 0xffffffffu;
   const int tid = threadIdx.x, J = tid & 31, K = tid >> 5;
   const Bte2Oct &O = P.oct[un.oct];
   const int ty = un.ty, tz = un.tz, b0 = un.b0;
   const int jp0 = ty * 64 + 2 * J, kp0 = tz * 2 * W + 2 * K;
-  const bool vk[2] = {kp0 < P.nz, kp0 + 1 < P.nz};
-  const bool vthread = (jp0 < P.ny) && vk[0];
-  const int jl = min(P.ny, (ty + 1) * 64) - 1 - ty * 64, kl = min(P.nz, (tz + 1) * 2 * W) - 1 - tz * 2 * W;
-  const int Jl = jl >> 1, jjl = jl & 1, Kl = kl >> 1, kkl = kl & 1;
+  // ny and nz are even on this path (host check): a patch is valid or invalid as a whole, and the last
+  // valid row of a tile is always the jj = 1 / kk = 1 row of lane Jl / warp Kl
+  const bool vthread = (jp0 < P.ny) && (kp0 < P.nz);
+  const int Jl = (min(P.ny, (ty + 1) * 64) - 1 - ty * 64) >> 1, Kl = (min(P.nz, (tz + 1) * 2 * W) - 1 - tz * 2 * W) >> 1;
   const bool first = un.dep_prev < 0;                  // first band group of this octant: M is written, not added to
   const int ebase = P.epoch << 16;
 
   const Ch *xin = reinterpret_cast<const Ch *>(O.xin);
   Ch *xout = reinterpret_cast<Ch *>(O.xout);
-  Ch *ypl = reinterpret_cast<Ch *>(O.ypl);
-  Ch *zpl = reinterpret_cast<Ch *>(O.zpl);
   Bte2Mom<T> *M = reinterpret_cast<Bte2Mom<T> *>(O.M);
   const Bte2Pair<T> *dTQ = reinterpret_cast<const Bte2Pair<T> *>(P.dTQ[O.cls]);
 
-  // cell index of row (jj,kk) at step t: base[kk] + jj*32 + (t - K) * 64
+  // cell index of row (jj,kk) at step t: cbase[kk] + jj*32 + (t - K) * 64
   int64_t cbase[2];
 #pragma unroll
   for (int kk = 0; kk < 2; ++kk) {
-    const int kp = kp0 + kk, k = vk[kk] ? (O.sz > 0 ? kp : P.nz - 1 - kp) : 0;
-    cbase[kk] = (((int64_t)k * P.nty + ty) * P.NU) * 64 + J;
+    const int kp = kp0 + kk, k = vthread ? (O.sz > 0 ? kp : P.nz - 1 - kp) : 0;
+    cbase[kk] = (((int64_t)k * P.nty + ty) * P.NU) * 64 + J - (int64_t)K * 64;
   }
+  // plane pointers of this thread at step 0; all advance by a constant stride per step
+  //   z inflow staging: element e = tid + q*NT of the [b][jj][ch][lane] block of step u
+  const Ch *zsrc = reinterpret_cast<const Ch *>(O.zpl) + zpl2_index<T>(P, tz, ty, b0, 0, 0, 0, 0);
+  const int64_t zstep = 2 * NCH * 32, zband = (int64_t)P.NU * 2 * NCH * 32;
+  Ch *zdst = reinterpret_cast<Ch *>(O.zpl) + zpl2_index<T>(P, tz + 1, ty, b0, 0, 0, 0, 0);
+  //   y planes: lane l < 2*NC of warp K loads chunk (b, kk, ch) of the cell i' = t - K
+  const int yb = J / (2 * NCH), ykk = (J / NCH) & 1, ych = J % NCH;
+  const Ch *ysrc = reinterpret_cast<const Ch *>(O.ypl) + ypl2_index<T>(P, ty, tz, b0 + (J < 2 * NC ? yb : 0), K, 0, ykk, ych) - (int64_t)K * 2 * NCH;
+  Ch *ydst = reinterpret_cast<Ch *>(O.ypl) + ypl2_index<T>(P, ty + 1, tz, b0 + (J < 2 * NC ? yb : 0), K, 0, ykk, ych);
 
-  // ---- progress of the units this one follows (uniform; smem cache + poll by threads 0..2)
-  auto wait_deps = [&](int t) {
-    const int need0 = t + 33, need1 = t + 1 + W, need2 = t + 1;
-    if (S->cache[0] < need0 || S->cache[1] < need1 || S->cache[2] < need2) {
-      __syncthreads();
-      if (tid < 3) {
-        const int dep = tid == 0 ? un.dep_y : (tid == 1 ? un.dep_z : un.dep_prev);
-        const int need = tid == 0 ? need0 : (tid == 1 ? need1 : need2);
-        if (dep >= 0) {
-          int v;
-          while ((v = ld_acquire_gpu(P.prog + dep) - ebase) < need) __nanosleep(100);
-          S->cache[tid] = v;
-        }
+  // ---- progress of the units this one follows: lanes 0..2 of warp 0 keep the last value seen in a register
+  const int mydep = tid == 0 ? un.dep_y : (tid == 1 ? un.dep_z : (tid == 2 ? un.dep_prev : -1));
+  const int mylag = tid == 0 ? 33 : (tid == 1 ? W + 1 : 1);
+  int seen = 0, peek = 0;
+  auto ensure = [&](int t1) {          // everything step t1 reads from other units has been published
+    if (mydep >= 0 && !(P.dbg & 4)) {
+      seen = max(seen, peek - ebase);
+      if (seen < t1 + mylag) {
+        int v;
+        while ((v = ld_acquire_gpu(P.prog + mydep) - ebase) < t1 + mylag) __nanosleep(64);
+        seen = v;
       }
-      __syncthreads();
     }
   };
-  if (tid < 3) {
-    const int dep = tid == 0 ? un.dep_y : (tid == 1 ? un.dep_z : un.dep_prev);
-    S->cache[tid] = dep < 0 ? 0x7fffffff : 0;
-  }
-  __syncthreads();
-  wait_deps(-1);
 
-  // ---- asynchronous prefetch (global -> shared) of everything step t1 consumes
-  auto prefetch = [&](int t1, int par) {
-    // (dT, Q) of the four cells
+  // ---- previous content of the moment accumulator for step t1 (own commit group, one step ahead)
+  auto prefetch_m = [&](int t1) {
     const int ip1 = t1 - J - K;
-    if (vthread && ip1 >= 0 && ip1 < P.nx) {
+    if (!first && !(P.dbg & 2) && vthread && ip1 >= 0 && ip1 < P.nx) {
 #pragma unroll
       for (int kk = 0; kk < 2; ++kk)
-        if (vk[kk]) {
 #pragma unroll
-          for (int jj = 0; jj < 2; ++jj)
-            cp_async<sizeof(Bte2Pair<T>)>(&S->inp[par][kk][jj][tid], dTQ + cbase[kk] + jj * 32 + (int64_t)(t1 - K) * 64);
+        for (int jj = 0; jj < 2; ++jj) {
+          const int64_t ci = cbase[kk] + jj * 32 + (int64_t)t1 * 64;
+#pragma unroll
+          for (int h = 0; h < (int)sizeof(Bte2Mom<T>) / 16; ++h)
+            cp_async<16>(reinterpret_cast<char *>(&S->mold[t1 & 1][kk][jj][tid]) + 16 * h, reinterpret_cast<const char *>(M + ci) + 16 * h);
         }
     }
-    // z inflow plane of warp 0 -> zbuf slot 0
-    if (t1 < P.NU) {
+  };
+  // ---- outflow faces of step t1 (staged in shared memory by the step) -> global planes, coalesced
+  auto copy_out = [&](int t1) {
+    const int par = (t1 & 1) ^ 1;                      // buffer the step wrote
+    if (!(P.dbg & 1) && kp0 < P.nz) {
+      const int ipl = t1 - Jl - K;                     // cell lane Jl of this warp finished in step t1
+      if (J < 2 * NC && ipl >= 0 && ipl < P.nx) ydst[(int64_t)ipl * 2 * NCH] = S->yst[par][K][ykk * NC + yb * NCH + ych];
+    }
+    const int ul = t1 - Kl;
+    if (!(P.dbg & 1) && ul >= 0 && ul < P.NU) {
 #pragma unroll
       for (int q = 0; q < (2 * NC * 32) / NT; ++q) {
         const int e = tid + q * NT, b = e / (2 * NCH * 32), rem = e % (2 * NCH * 32);
-        const int jj = rem / (NCH * 32), ch = (rem / 32) % NCH, l = rem & 31;
-        cp_async<16>(&S->zbuf[par][0][jj][b * NCH + ch][l], zpl + zpl2_index<T>(P, tz, ty, b0 + b, t1, 0, 0, 0) + rem);
+        zdst[b * zband + ul * zstep + rem] = (&S->zex[par][Kl][0][b * NCH][0])[(rem / (NCH * 32)) * (NC * 32) + (rem % (NCH * 32))];
       }
     }
-    // y inflow of lane 0 of every warp -> ybuf
+  };
+  // ---- asynchronous prefetch (global -> shared) of everything step t1 consumes
+  auto prefetch = [&](int t1) {
+    const int rb = t1 % R;
+    const int ip1 = t1 - J - K;
+    if (vthread && ip1 >= 0 && ip1 < P.nx) {
+#pragma unroll
+      for (int kk = 0; kk < 2; ++kk) {
+#pragma unroll
+          for (int jj = 0; jj < 2; ++jj) {
+            const int64_t ci = cbase[kk] + jj * 32 + (int64_t)t1 * 64;
+            cp_async<sizeof(Bte2Pair<T>)>(&S->inp[rb][kk][jj][tid], dTQ + ci);
+          }
+        }
+    }
+    if (t1 < P.NU && !(P.dbg & 8)) {
+#pragma unroll
+      for (int q = 0; q < (2 * NC * 32) / NT; ++q) {
+        const int e = tid + q * NT, b = e / (2 * NCH * 32), rem = e % (2 * NCH * 32);
+        cp_async<16>(&S->zin0[rb][0][b * NCH][0] + (rem / (NCH * 32)) * (NC * 32) + (rem % (NCH * 32)), zsrc + b * zband + t1 * zstep + rem);
+      }
+    }
     {
       const int ipy = t1 - K;
-      if (J < 2 * NC && ipy >= 0 && ipy < P.nx) {
-        const int b = J / (2 * NCH), kk = (J / NCH) & 1, ch = J % NCH;
-        cp_async<16>(&S->ybuf[par][K][kk][b * NCH + ch], ypl + ypl2_index<T>(P, ty, tz, b0 + b, K, ipy, kk, ch));
-      }
+      if (J < 2 * NC && ipy >= 0 && ipy < P.nx) cp_async<16>(&S->ybuf[rb][K][ykk][yb * NCH + ych], ysrc + (int64_t)t1 * 2 * NCH);
     }
   };
 
@@ -248,34 +279,74 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
           for (int q = 0; q < CP; ++q) c[jj][kk][b * BTE2_P + ch * CP + q] = v.v[q];
         }
 
-  prefetch(0, 0);
-  cp_async_wait_all();
+  ensure(D + BTE2_SLACK);
+  __syncthreads();
+#pragma unroll
+  for (int t1 = 0; t1 < D; ++t1) {
+    if (t1 == 0) prefetch_m(0);
+    prefetch(t1); cp_async_commit();
+  }
+  cp_async_wait<D - 1>();
   __syncthreads();
 
   T bcx[NB], bcy[NB];
 #pragma unroll
   for (int b = 0; b < NB; ++b) { bcx[b] = CF.bc[b0 + b][0]; bcy[b] = CF.bc[b0 + b][1]; }
 
+  // one (band, chunk) of the 2x2 patch: FAST = every lane of the warp is active (no predication)
+  auto chunk = [&](auto fastc, int b, int ch, const T (&r)[2][2], T (&m)[2][2][4], int rb, int cur, bool act) {
+    constexpr bool FAST = decltype(fastc)::value;
+    const int q0 = b * BTE2_P + ch * CP, cn = b * NCH + ch;
+    // y inflow: lane J-1's jj=1 rows of the previous step; lane 0: the staged plane
+    T yin[2][CP];
+#pragma unroll
+    for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+      for (int q = 0; q < CP; ++q) yin[kk][q] = shfl_up1<T>(c[1][kk][q0 + q]);
+    if (J == 0) {
+#pragma unroll
+      for (int kk = 0; kk < 2; ++kk) {
+        const Ch v = S->ybuf[rb][K][kk][cn];
+#pragma unroll
+        for (int q = 0; q < CP; ++q) yin[kk][q] = v.v[q];
+      }
+    }
+    // z inflow: warp K-1's kk=1 rows of the previous step, or the staged plane for warp 0
+    const Ch *zp = K == 0 ? &S->zin0[rb][0][cn][J] : &S->zex[cur][K - 1][0][cn][J];
+    const Ch z0 = zp[0], z1 = zp[NC * 32];
+    if (FAST || act) {
+      Ch o0, o1;
+#pragma unroll
+      for (int q = 0; q < CP; ++q) {
+        const int p = ch * CP + q;
+        const T inv = CF.k[b0 + b][p][0], ax = CF.k[b0 + b][p][1], ay = CF.k[b0 + b][p][2], az = CF.k[b0 + b][p][3];
+        const T w0 = CF.k[b0 + b][p][4], w1 = CF.k[b0 + b][p][5], w2 = CF.k[b0 + b][p][6], w3 = CF.k[b0 + b][p][7];
+        T e00 = r[0][0] * inv; e00 = fma(ax, c[0][0][q0 + q], e00); e00 = fma(ay, yin[0][q], e00); e00 = fma(az, z0.v[q], e00);
+        T e10 = r[1][0] * inv; e10 = fma(ax, c[1][0][q0 + q], e10); e10 = fma(az, z1.v[q], e10); e10 = fma(ay, e00, e10);
+        T e01 = r[0][1] * inv; e01 = fma(ax, c[0][1][q0 + q], e01); e01 = fma(ay, yin[1][q], e01); e01 = fma(az, e00, e01);
+        T e11 = r[1][1] * inv; e11 = fma(ax, c[1][1][q0 + q], e11); e11 = fma(ay, e01, e11); e11 = fma(az, e10, e11);
+        c[0][0][q0 + q] = e00; c[1][0][q0 + q] = e10; c[0][1][q0 + q] = e01; c[1][1][q0 + q] = e11;
+        o0.v[q] = e01; o1.v[q] = e11;
+        m[0][0][0] = fma(w0, e00, m[0][0][0]); m[0][0][1] = fma(w1, e00, m[0][0][1]); m[0][0][2] = fma(w2, e00, m[0][0][2]); m[0][0][3] = fma(w3, e00, m[0][0][3]);
+        m[1][0][0] = fma(w0, e10, m[1][0][0]); m[1][0][1] = fma(w1, e10, m[1][0][1]); m[1][0][2] = fma(w2, e10, m[1][0][2]); m[1][0][3] = fma(w3, e10, m[1][0][3]);
+        m[0][1][0] = fma(w0, e01, m[0][1][0]); m[0][1][1] = fma(w1, e01, m[0][1][1]); m[0][1][2] = fma(w2, e01, m[0][1][2]); m[0][1][3] = fma(w3, e01, m[0][1][3]);
+        m[1][1][0] = fma(w0, e11, m[1][1][0]); m[1][1][1] = fma(w1, e11, m[1][1][1]); m[1][1][2] = fma(w2, e11, m[1][1][2]); m[1][1][3] = fma(w3, e11, m[1][1][3]);
+      }
+      Ch *zo = &S->zex[cur ^ 1][K][0][cn][J];
+      zo[0] = o0; zo[NC * 32] = o1;
+    }
+  };
+
   for (int t = 0; t < P.nsteps; ++t) {
-    const int cur = t & 1, nxt = cur ^ 1;
+    const int cur = t & 1, rb = t % R;
     const int ip = t - J - K;
     const bool act = vthread && ip >= 0 && ip < P.nx;
-    wait_deps(t);
-    // previous content of the moment accumulator (this step) + everything step t+1 reads
-    if (act && !first) {
-#pragma unroll
-      for (int kk = 0; kk < 2; ++kk)
-        if (vk[kk]) {
-#pragma unroll
-          for (int jj = 0; jj < 2; ++jj) {
-            const Bte2Mom<T> *src = M + cbase[kk] + jj * 32 + (int64_t)(t - K) * 64;
-#pragma unroll
-            for (int h = 0; h < (int)sizeof(Bte2Mom<T>) / 16; ++h)
-              cp_async<16>(reinterpret_cast<char *>(&S->mold[kk][jj][tid]) + 16 * h, reinterpret_cast<const char *>(src) + 16 * h);
-          }
-        }
-    }
-    prefetch(t + 1, nxt);
+    prefetch_m(t + 1);
+    cp_async_commit();
+    prefetch(t + D);
+    cp_async_commit();
+    if (t > 0) copy_out(t - 1);
+    if (tid < 3 && mydep >= 0 && seen < t + 1 + D + mylag) peek = ld_acquire_gpu(P.prog + mydep);   // consumed by ensure() below
 
     T m[2][2][4];
 #pragma unroll
@@ -289,8 +360,9 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
 #pragma unroll
     for (int kk = 0; kk < 2; ++kk)
 #pragma unroll
-      for (int jj = 0; jj < 2; ++jj) in[jj][kk] = S->inp[cur][kk][jj][tid];
+      for (int jj = 0; jj < 2; ++jj) in[jj][kk] = S->inp[rb][kk][jj][tid];
 
+    const bool fast = __all_sync(FULL, act);
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
       T r[2][2];
@@ -298,55 +370,20 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
       for (int kk = 0; kk < 2; ++kk)
 #pragma unroll
         for (int jj = 0; jj < 2; ++jj) r[jj][kk] = fma(bcx[b], in[jj][kk].x, bcy[b] * in[jj][kk].y);
+      if (fast) {
 #pragma unroll
-      for (int ch = 0; ch < NCH; ++ch) {
-        const int q0 = b * BTE2_P + ch * CP, cn = b * NCH + ch;
-        // y inflow: lane J-1's jj=1 rows of the previous step; lane 0: the staged plane
-        T yin[2][CP];
+        for (int ch = 0; ch < NCH; ++ch) chunk(std::true_type{}, b, ch, r, m, rb, cur, true);
+      } else {
 #pragma unroll
-        for (int kk = 0; kk < 2; ++kk)
-#pragma unroll
-          for (int q = 0; q < CP; ++q) yin[kk][q] = shfl_up1<T>(c[1][kk][q0 + q]);
-        if (J == 0) {
-#pragma unroll
-          for (int kk = 0; kk < 2; ++kk) {
-            const Ch v = S->ybuf[cur][K][kk][cn];
-#pragma unroll
-            for (int q = 0; q < CP; ++q) yin[kk][q] = v.v[q];
-          }
-        }
-        // z inflow: slot K (warp K-1's kk=1 rows of the previous step, or the staged plane)
-        const Ch z0 = S->zbuf[cur][K][0][cn][J], z1 = S->zbuf[cur][K][1][cn][J];
-        if (act) {
-          Ch o0, o1;
-#pragma unroll
-          for (int q = 0; q < CP; ++q) {
-            const int p = ch * CP + q;
-            const T inv = CF.k[b0 + b][p][0], ax = CF.k[b0 + b][p][1], ay = CF.k[b0 + b][p][2], az = CF.k[b0 + b][p][3];
-            const T w0 = CF.k[b0 + b][p][4], w1 = CF.k[b0 + b][p][5], w2 = CF.k[b0 + b][p][6], w3 = CF.k[b0 + b][p][7];
-            T e00 = r[0][0] * inv; e00 = fma(ax, c[0][0][q0 + q], e00); e00 = fma(ay, yin[0][q], e00); e00 = fma(az, z0.v[q], e00);
-            T e10 = r[1][0] * inv; e10 = fma(ax, c[1][0][q0 + q], e10); e10 = fma(az, z1.v[q], e10); e10 = fma(ay, e00, e10);
-            T e01 = r[0][1] * inv; e01 = fma(ax, c[0][1][q0 + q], e01); e01 = fma(ay, yin[1][q], e01); e01 = fma(az, e00, e01);
-            T e11 = r[1][1] * inv; e11 = fma(ax, c[1][1][q0 + q], e11); e11 = fma(ay, e01, e11); e11 = fma(az, e10, e11);
-            c[0][0][q0 + q] = e00; c[1][0][q0 + q] = e10; c[0][1][q0 + q] = e01; c[1][1][q0 + q] = e11;
-            o0.v[q] = e01; o1.v[q] = e11;
-            m[0][0][0] = fma(w0, e00, m[0][0][0]); m[0][0][1] = fma(w1, e00, m[0][0][1]); m[0][0][2] = fma(w2, e00, m[0][0][2]); m[0][0][3] = fma(w3, e00, m[0][0][3]);
-            m[1][0][0] = fma(w0, e10, m[1][0][0]); m[1][0][1] = fma(w1, e10, m[1][0][1]); m[1][0][2] = fma(w2, e10, m[1][0][2]); m[1][0][3] = fma(w3, e10, m[1][0][3]);
-            m[0][1][0] = fma(w0, e01, m[0][1][0]); m[0][1][1] = fma(w1, e01, m[0][1][1]); m[0][1][2] = fma(w2, e01, m[0][1][2]); m[0][1][3] = fma(w3, e01, m[0][1][3]);
-            m[1][1][0] = fma(w0, e11, m[1][1][0]); m[1][1][1] = fma(w1, e11, m[1][1][1]); m[1][1][2] = fma(w2, e11, m[1][1][2]); m[1][1][3] = fma(w3, e11, m[1][1][3]);
-          }
-          S->zbuf[nxt][K + 1][0][cn][J] = o0;
-          S->zbuf[nxt][K + 1][1][cn][J] = o1;
-        }
+        for (int ch = 0; ch < NCH; ++ch) chunk(std::false_type{}, b, ch, r, m, rb, cur, act);
       }
     }
 
-    cp_async_wait_all();                 // mold of this step and the planes / inputs of the next one have landed
     if (act) {
       // (b) moments of this band group into the octant accumulator (one owner per cell and group)
 #pragma unroll
       for (int kk = 0; kk < 2; ++kk)
-        if (vk[kk]) {
+        if (!(P.dbg & 2)) {
 #pragma unroll
           for (int jj = 0; jj < 2; ++jj) {
             Bte2Mom<T> o;
@@ -354,14 +391,14 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
 #pragma unroll
               for (int q = 0; q < 4; ++q) o.v[q] = m[jj][kk][q];
             } else {
-              const Bte2Mom<T> old = S->mold[kk][jj][tid];
+              const Bte2Mom<T> old = S->mold[cur][kk][jj][tid];
 #pragma unroll
               for (int q = 0; q < 4; ++q) o.v[q] = old.v[q] + m[jj][kk][q];
             }
-            M[cbase[kk] + jj * 32 + (int64_t)(t - K) * 64] = o;
+            M[cbase[kk] + jj * 32 + (int64_t)t * 64] = o;
           }
         }
-      // outflow faces: tile hand-off / lagged boundary store
+      // y outflow rows (jj = 1 of lane Jl) -> staging buffer; written to the plane by copy_out() next step
       if (J == Jl) {
 #pragma unroll
         for (int b = 0; b < NB; ++b)
@@ -371,30 +408,21 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
             for (int ch = 0; ch < NCH; ++ch) {
               Ch o;
 #pragma unroll
-              for (int q = 0; q < CP; ++q) o.v[q] = jjl ? c[1][kk][b * BTE2_P + ch * CP + q] : c[0][kk][b * BTE2_P + ch * CP + q];
-              ypl[ypl2_index<T>(P, ty + 1, tz, b0 + b, K, ip, kk, ch)] = o;
-            }
-      }
-      if (K == Kl) {
-#pragma unroll
-        for (int b = 0; b < NB; ++b)
-#pragma unroll
-          for (int jj = 0; jj < 2; ++jj)
-#pragma unroll
-            for (int ch = 0; ch < NCH; ++ch) {
-              Ch o;
-#pragma unroll
-              for (int q = 0; q < CP; ++q) o.v[q] = kkl ? c[jj][1][b * BTE2_P + ch * CP + q] : c[jj][0][b * BTE2_P + ch * CP + q];
-              zpl[zpl2_index<T>(P, tz + 1, ty, b0 + b, t - K, jj, ch, J)] = o;
+              for (int q = 0; q < CP; ++q) o.v[q] = c[1][kk][b * BTE2_P + ch * CP + q];
+              S->yst[cur ^ 1][K][kk * NC + b * NCH + ch] = o;
             }
       }
     }
+    cp_async_wait<D - 1>();            // everything step t+1 reads has landed
+    if (tid < 3) ensure(t + 1 + D);    // ... and what step t+1 prefetches has been published upstream
     __syncthreads();
-    if ((t & (BTE2_PUB - 1)) == BTE2_PUB - 1 && tid == 0) {
+    if ((t & (BTE2_PUB - 1)) == BTE2_PUB - 1 && tid == 0) {   // faces and moments of steps < t are in global memory
       __threadfence();
-      st_release_gpu(P.prog + unit, ebase + t + 1);
+      st_release_gpu(P.prog + unit, ebase + t);
     }
   }
+  cp_async_wait<0>();
+  copy_out(P.nsteps - 1);
 
   // ---- x outflow (carries are final: a thread stops updating them after its last active step)
 #pragma unroll
@@ -419,7 +447,7 @@ template <typename T, int W>
 __global__ void __launch_bounds__(W * 32) bte2_sweep_kernel(const __grid_constant__ Bte2Dev P,
                                                             const __grid_constant__ Bte2Coefs<T> CF) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  constexpr int NBMAX = sizeof(T) == 4 ? 2 : 1;
+  constexpr int NBMAX = sizeof(T) == 4 ? 2 : 1, D = BTE2_DIST;
   __shared__ int s_unit;
   for (;;) {
     __syncthreads();
@@ -428,8 +456,8 @@ __global__ void __launch_bounds__(W * 32) bte2_sweep_kernel(const __grid_constan
     const int unit = s_unit;
     if (unit >= P.n_units) break;
     const Bte2Unit un = P.units[unit];
-    if (NBMAX == 2 && un.nb == 2) bte2_run_unit<T, NBMAX, W>(P, CF, un, smem_raw, unit);
-    else bte2_run_unit<T, 1, W>(P, CF, un, smem_raw, unit);
+    if (NBMAX == 2 && un.nb == 2) bte2_run_unit<T, NBMAX, W, D>(P, CF, un, smem_raw, unit);
+    else bte2_run_unit<T, 1, W, D>(P, CF, un, smem_raw, unit);
   }
 }
 
