@@ -32,7 +32,7 @@ BTE_FP64, BTE_FP32_STORE_FP64_ACC = 0, 1
 EXPORTS = ["bte_workspace_bytes", "bte_create", "bte_iterate", "bte_get_temperature", "bte_get_heat_flux",
            "bte_set_temperature", "bte_residual", "bte_solve_host", "bte_set_sweep_timing",
            "bte_get_sweep_timing", "bte_updates_per_sweep",
-           "bte_iterations_done", "bte_kernel_launches_per_iteration", "bte_schedule_info", "bte_destroy",
+           "bte_iterations_done", "bte_kernel_launches_per_iteration", "bte_kernel_path", "bte_schedule_info", "bte_destroy",
            "bte_status_string", "bte_last_cuda_error"]
 
 
@@ -99,6 +99,8 @@ def lib():
         L.bte_iterations_done.restype = i64
         L.bte_kernel_launches_per_iteration.argtypes = [vp]
         L.bte_kernel_launches_per_iteration.restype = i32
+        L.bte_kernel_path.argtypes = [vp]
+        L.bte_kernel_path.restype = i32
         L.bte_schedule_info.argtypes = [vp, C.POINTER(i64)]
         L.bte_schedule_info.restype = None
         L.bte_destroy.argtypes = [vp]
@@ -248,6 +250,10 @@ class Solver:
     @property
     def launches_per_iteration(self):
         return int(lib().bte_kernel_launches_per_iteration(self.h))
+
+    @property
+    def kernel_path(self):
+        return int(lib().bte_kernel_path(self.h))
 
     def schedule_info(self):
         out = (C.c_int64 * 6)()

@@ -762,6 +762,7 @@ int64_t bte_updates_per_sweep(const bte_solver *h) {
 }
 int64_t bte_iterations_done(const bte_solver *h) { return h ? h->iters : 0; }
 int32_t bte_kernel_launches_per_iteration(const bte_solver *h) { return h ? h->launches_per_iter : 0; }
+int32_t bte_kernel_path(const bte_solver *h) { return h ? (h->pl.v2 ? 2 : 1) : 0; }
 
 void bte_schedule_info(const bte_solver *h, int64_t out[6]) {
   if (!h || !out) return;

@@ -294,7 +294,8 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
   for (int b = 0; b < NB; ++b) { bcx[b] = CF.bc[b0 + b][0]; bcy[b] = CF.bc[b0 + b][1]; }
 
   // one (band, chunk) of the 2x2 patch: FAST = every lane of the warp is active (no predication)
-  auto chunk = [&](auto fastc, int b, int ch, const T (&r)[2][2], T (&m)[2][2][4], int rb, int cur, bool act) {
+  auto chunk = [&](auto fastc, int b, int ch, const T (&r)[2][2], T (&m)[2][2][4], int rb, int cur, bool act,
+                   const Ch *__restrict__ zrd, Ch *__restrict__ zwr) {
     constexpr bool FAST = decltype(fastc)::value;
     const int q0 = b * BTE2_P + ch * CP, cn = b * NCH + ch;
     // y inflow: lane J-1's jj=1 rows of the previous step; lane 0: the staged plane
@@ -312,8 +313,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
       }
     }
     // z inflow: warp K-1's kk=1 rows of the previous step, or the staged plane for warp 0
-    const Ch *zp = K == 0 ? &S->zin0[rb][0][cn][J] : &S->zex[cur][K - 1][0][cn][J];
-    const Ch z0 = zp[0], z1 = zp[NC * 32];
+    const Ch z0 = zrd[cn * 32], z1 = zrd[(NC + cn) * 32];
     if (FAST || act) {
       Ch o0, o1;
 #pragma unroll
@@ -332,8 +332,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
         m[0][1][0] = fma(w0, e01, m[0][1][0]); m[0][1][1] = fma(w1, e01, m[0][1][1]); m[0][1][2] = fma(w2, e01, m[0][1][2]); m[0][1][3] = fma(w3, e01, m[0][1][3]);
         m[1][1][0] = fma(w0, e11, m[1][1][0]); m[1][1][1] = fma(w1, e11, m[1][1][1]); m[1][1][2] = fma(w2, e11, m[1][1][2]); m[1][1][3] = fma(w3, e11, m[1][1][3]);
       }
-      Ch *zo = &S->zex[cur ^ 1][K][0][cn][J];
-      zo[0] = o0; zo[NC * 32] = o1;
+      zwr[cn * 32] = o0; zwr[(NC + cn) * 32] = o1;
     }
   };
 
@@ -363,6 +362,8 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
       for (int jj = 0; jj < 2; ++jj) in[jj][kk] = S->inp[rb][kk][jj][tid];
 
     const bool fast = __all_sync(FULL, act);
+    const Ch *__restrict__ zrd = K == 0 ? &S->zin0[rb][0][0][J] : &S->zex[cur][K - 1][0][0][J];
+    Ch *__restrict__ zwr = &S->zex[cur ^ 1][K][0][0][J];
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
       T r[2][2];
@@ -372,10 +373,10 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
         for (int jj = 0; jj < 2; ++jj) r[jj][kk] = fma(bcx[b], in[jj][kk].x, bcy[b] * in[jj][kk].y);
       if (fast) {
 #pragma unroll
-        for (int ch = 0; ch < NCH; ++ch) chunk(std::true_type{}, b, ch, r, m, rb, cur, true);
+        for (int ch = 0; ch < NCH; ++ch) chunk(std::true_type{}, b, ch, r, m, rb, cur, true, zrd, zwr);
       } else {
 #pragma unroll
-        for (int ch = 0; ch < NCH; ++ch) chunk(std::false_type{}, b, ch, r, m, rb, cur, act);
+        for (int ch = 0; ch < NCH; ++ch) chunk(std::false_type{}, b, ch, r, m, rb, cur, act, zrd, zwr);
       }
     }
 

@@ -75,15 +75,41 @@ def check(bte, p, n, precision=None, checkpoints=(), res_rtol=None):
 
 # ---------------------------------------------------------------- shrunken configs (T2)
 SHRUNK = {0: (57, 1, 1), 1: (45, 70, 1), 2: (19, 37, 21), 3: (40, 36, 32), 4: (43, 34, 19)}
+# even ny, nz: served by the fast path (tiles of 64 x 8/16 rows: ragged in y and z, two tiles in y for 4')
+SHRUNK_FAST = {2: (21, 38, 22), 4: (45, 130, 36)}
 
 
 @pytest.mark.parametrize("k", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("prec", [W.FP64, W.FP32_STORE_FP64_ACC])
 def test_shrunken_configs(bte, k, prec):
     """Every config at a size that spans several tiles with a ragged tail on every axis
-    (tiles are 32 rows in y and 8/16 in z), checked at n = 1, 2, 10, 30."""
+    (generic path: tiles are 32 rows in y and 8/16 in z), checked at n = 1, 2, 10, 30."""
     p = W.config(k, grid=SHRUNK[k])
     check(bte, p, 30, precision=prec, checkpoints=(1, 2, 10))
+
+
+@pytest.mark.parametrize("k", [2, 4])
+@pytest.mark.parametrize("prec", [W.FP64, W.FP32_STORE_FP64_ACC])
+def test_shrunken_configs_fast_path(bte, k, prec, monkeypatch):
+    """The 3-D unmasked configs on the fast sweep kernel, and the same problem forced onto the generic one."""
+    p = W.config(k, grid=SHRUNK_FAST[k])
+    assert bte.Solver(p, precision=prec).kernel_path == 2
+    check(bte, p, 30, precision=prec, checkpoints=(1, 2, 10))
+    monkeypatch.setenv("BTE_FORCE_GENERIC", "1")
+    assert bte.Solver(p, precision=prec).kernel_path == 1
+    check(bte, p, 6, precision=prec, checkpoints=(1,))
+
+
+@pytest.mark.parametrize("warps", ["4", "8"])
+def test_fast_path_tile_heights(bte, warps, monkeypatch):
+    """Both CTA shapes of the fast path (tiles of 8 and 16 rows in z), several z tiles, periodic + specular faces."""
+    monkeypatch.setenv("BTE_V2_W", warps)
+    p = W.config(4, grid=(37, 66, 52))
+    p.face_bc = [(W.BC_PERIODIC, 0.0), (W.BC_PERIODIC, 0.0), (W.BC_SPECULAR, 0.0), (W.BC_DIFFUSE, 0.0),
+                 (W.BC_ISOTHERMAL, 0.1), (W.BC_SPECULAR, 0.0)]
+    assert bte.Solver(p).kernel_path == 2
+    check(bte, p, 12, checkpoints=(1, 3))
+    check(bte, p, 4, precision=W.FP64)
 
 
 # ---------------------------------------------------------------- random problems: every BC mix
@@ -100,10 +126,12 @@ def test_random_masked_problems(bte, seed, dim):
 @pytest.mark.parametrize("bc", [W.BC_ISOTHERMAL, W.BC_DIFFUSE, W.BC_SPECULAR, W.BC_PERIODIC])
 def test_each_bc_type_alone(bte, bc):
     """One BC type on all side faces, z- isothermal so a steady state exists."""
-    p = W.config(2, grid=(33, 34, 9))
-    fb = [(bc, 0.25 if bc == W.BC_ISOTHERMAL else 0.0)] * 4 + [(W.BC_ISOTHERMAL, -0.3), (W.BC_DIFFUSE, 0.0)]
-    p.face_bc = fb
-    check(bte, p, 15, precision=W.FP64, checkpoints=(1, 2))
+    for grid in ((33, 34, 9), (33, 34, 10)):          # generic path / fast path
+        p = W.config(2, grid=grid)
+        fb = [(bc, 0.25 if bc == W.BC_ISOTHERMAL else 0.0)] * 4 + [(W.BC_ISOTHERMAL, -0.3), (W.BC_DIFFUSE, 0.0)]
+        p.face_bc = fb
+        assert bte.Solver(p).kernel_path == (2 if grid[2] % 2 == 0 else 1)
+        check(bte, p, 15, precision=W.FP64, checkpoints=(1, 2))
 
 
 def test_periodic_wrap_onto_void_uses_interface_bc(bte):
@@ -123,8 +151,9 @@ def test_single_cell_and_tiny_grids(bte):
         check(bte, p, 6, precision=W.FP64, checkpoints=(1,))
 
 
-def test_zero_iterations_and_zero_source(bte):
-    p = W.config(2, grid=(9, 8, 7))
+@pytest.mark.parametrize("grid", [(9, 8, 7), (10, 8, 8)])          # generic / fast path
+def test_zero_iterations_and_zero_source(bte, grid):
+    p = W.config(2, grid=grid)
     g = bte.Solver(p)
     g.iterate(0)
     assert g.iterations_done == 0
@@ -139,9 +168,10 @@ def test_zero_iterations_and_zero_source(bte):
     assert g.residual() == (0.0, 0.0)          # 0/0 -> 0 (reading G11)
 
 
-def test_set_temperature_restart(bte):
+@pytest.mark.parametrize("grid", [(17, 9, 11), (18, 10, 12)])      # generic / fast path
+def test_set_temperature_restart(bte, grid):
     import oracle
-    p = W.config(2, grid=(17, 9, 11))
+    p = W.config(2, grid=grid)
     rng = np.random.default_rng(7)
     dT0 = rng.uniform(-1, 1, size=(p.nz, p.ny, p.nx))
     ref = oracle.RefSolver(p); ref.set_temperature(dT0); ref.iterate(1)
@@ -150,16 +180,18 @@ def test_set_temperature_restart(bte):
     assert eT <= 1e-10 and eq <= 1e-10
 
 
-def test_bitwise_deterministic(bte):
-    p = W.config(3, grid=(24, 40, 24))
+@pytest.mark.parametrize("k", [3, 4])                               # generic (masked) / fast path
+def test_bitwise_deterministic(bte, k):
+    p = W.config(k, grid=(24, 40, 24))
     a = bte.Solver(p); a.iterate(7)
     b = bte.Solver(p); b.iterate(3); b.iterate(4)
     assert (a.temperature() == b.temperature()).all()
     assert (a.heat_flux() == b.heat_flux()).all()
 
 
-def test_solve_host_matches_device_path(bte):
-    p = W.config(2, grid=(20, 12, 9))
+@pytest.mark.parametrize("grid", [(20, 12, 9), (20, 12, 10)])      # generic / fast path
+def test_solve_host_matches_device_path(bte, grid):
+    p = W.config(2, grid=grid)
     g = bte.Solver(p); g.iterate(5)
     h = bte.Solver(p)
     dT, q = h.solve_host(np.ascontiguousarray(p.Q), 5)
