@@ -307,7 +307,7 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
       for (int q = 0; q < BTE2_P; ++q) {
         const double *r = blk + q * BTE_NCOEF;
         double k[8] = {r[0], r[1], r[2], r[3], r[4] / p->tau[b], p->v[b] * r[5], p->v[b] * r[6], p->v[b] * r[7]};
-        for (int c = 0; c < 8; ++c) { pl.cf64.k[b][q][c] = k[c]; pl.cf32.k[b][q][c] = (float)k[c]; }
+        for (int c = 0; c < 8; ++c) { pl.cf64.k[b][c][q] = k[c]; pl.cf32.k[b][c][q] = (float)k[c]; }
         if (b == 0) for (int a = 0; a < 3; ++a) d.wsa[q][a] = r[5 + a];
       }
       pl.cf64.bc[b][0] = pl.band[b]; pl.cf64.bc[b][1] = pl.band[B + b];

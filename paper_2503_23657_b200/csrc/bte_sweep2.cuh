@@ -34,7 +34,7 @@
 #define BTE2_TYROWS 64    // tile rows along y' (32 lanes x 2)
 
 template <typename T> struct alignas(16) Bte2Coefs {   // kernel parameter (constant bank 0)
-  T k[BTE2_MAXB][BTE2_P][8];   // inv, ax, ay, az, w/tau, v w|sx|, v w|sy|, v w|sz|
+  T k[BTE2_MAXB][8][BTE2_P];   // [band][inv, ax, ay, az, w/tau, v w|sx|, v w|sy|, v w|sz|][direction]
   T bc[BTE2_MAXB][2];          // C/4pi, C tau/(4pi sumC)
 };
 
@@ -131,6 +131,20 @@ template <typename T> __device__ __forceinline__ Bte2Chunk<T> ldcg_chunk(const B
   memcpy(&r, &v, 16);
   return r;
 }
+// packed pairs of directions: fp32 uses the sm_100 two-wide FMA (FFMA2: two FMAs per issue slot, so the
+// non-FMA instructions of the step issue in the shadow of the FMA pipe); fp64 is two scalar DFMAs
+template <typename T> struct Bte2V2;
+template <> struct Bte2V2<float> { typedef float2 t; };
+template <> struct Bte2V2<double> { typedef double2 t; };
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ double2 fma2(double2 a, double2 b, double2 c) { return make_double2(fma(a.x, b.x, c.x), fma(a.y, b.y, c.y)); }
+__device__ __forceinline__ double2 mul2(double2 a, double2 b) { return make_double2(a.x * b.x, a.y * b.y); }
+// moment accumulation m += w * e over a pair: fp32 keeps even / odd partial sums (one FFMA2), fp64 one sum
+__device__ __forceinline__ void acc2(float2 &m, float2 w, float2 e) { m = __ffma2_rn(w, e, m); }
+__device__ __forceinline__ void acc2(double2 &m, double2 w, double2 e) { m.x = fma(w.x, e.x, m.x); m.x = fma(w.y, e.y, m.x); }
+__device__ __forceinline__ float2 mk2(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ double2 mk2(double a, double b) { return make_double2(a, b); }
 template <typename T> __device__ __forceinline__ T shfl_up1(T v);
 template <> __device__ __forceinline__ float shfl_up1<float>(float v) { return __shfl_up_sync(0xffffffffu, v, 1); }
 template <> __device__ __forceinline__ double shfl_up1<double>(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
@@ -265,7 +279,8 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
   };
 
   // ---- x inflow -> carry registers (kept untouched by a thread until its first active step)
-  T c[2][2][NB * BTE2_P];                             // [jj][kk][b*16 + p]
+  typedef typename Bte2V2<T>::t V2;
+  V2 c[2][2][NB * BTE2_P / 2];                        // [jj][kk][(b*16 + p) / 2]: pairs of directions
 #pragma unroll
   for (int kk = 0; kk < 2; ++kk)
 #pragma unroll
@@ -276,7 +291,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
         for (int ch = 0; ch < NCH; ++ch) {
           const Ch v = ldcg_chunk<T>(xin + xpl2_index<T>(P, ty, tz, b0 + b, K, kk, jj, ch, J));
 #pragma unroll
-          for (int q = 0; q < CP; ++q) c[jj][kk][b * BTE2_P + ch * CP + q] = v.v[q];
+          for (int q = 0; q < CP; q += 2) c[jj][kk][(b * BTE2_P + ch * CP + q) / 2] = mk2(v.v[q], v.v[q + 1]);
         }
 
   ensure(D + BTE2_SLACK);
@@ -294,22 +309,23 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
   for (int b = 0; b < NB; ++b) { bcx[b] = CF.bc[b0 + b][0]; bcy[b] = CF.bc[b0 + b][1]; }
 
   // one (band, chunk) of the 2x2 patch: FAST = every lane of the warp is active (no predication)
-  auto chunk = [&](auto fastc, int b, int ch, const T (&r)[2][2], T (&m)[2][2][4], int rb, int cur, bool act,
+  auto chunk = [&](auto fastc, int b, int ch, const V2 (&r)[2][2], V2 (&m)[2][2][4], int rb, int cur, bool act,
                    const Ch *__restrict__ zrd, Ch *__restrict__ zwr) {
     constexpr bool FAST = decltype(fastc)::value;
-    const int q0 = b * BTE2_P + ch * CP, cn = b * NCH + ch;
+    constexpr int NP = CP / 2;                         // direction pairs per chunk
+    const int h0 = (b * BTE2_P + ch * CP) / 2, cn = b * NCH + ch;
     // y inflow: lane J-1's jj=1 rows of the previous step; lane 0: the staged plane
-    T yin[2][CP];
+    V2 yin[2][NP];
 #pragma unroll
     for (int kk = 0; kk < 2; ++kk)
 #pragma unroll
-      for (int q = 0; q < CP; ++q) yin[kk][q] = shfl_up1<T>(c[1][kk][q0 + q]);
+      for (int q = 0; q < NP; ++q) yin[kk][q] = mk2(shfl_up1<T>(c[1][kk][h0 + q].x), shfl_up1<T>(c[1][kk][h0 + q].y));
     if (J == 0) {
 #pragma unroll
       for (int kk = 0; kk < 2; ++kk) {
         const Ch v = S->ybuf[rb][K][kk][cn];
 #pragma unroll
-        for (int q = 0; q < CP; ++q) yin[kk][q] = v.v[q];
+        for (int q = 0; q < NP; ++q) yin[kk][q] = mk2(v.v[2 * q], v.v[2 * q + 1]);
       }
     }
     // z inflow: warp K-1's kk=1 rows of the previous step, or the staged plane for warp 0
@@ -317,20 +333,24 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     if (FAST || act) {
       Ch o0, o1;
 #pragma unroll
-      for (int q = 0; q < CP; ++q) {
-        const int p = ch * CP + q;
-        const T inv = CF.k[b0 + b][p][0], ax = CF.k[b0 + b][p][1], ay = CF.k[b0 + b][p][2], az = CF.k[b0 + b][p][3];
-        const T w0 = CF.k[b0 + b][p][4], w1 = CF.k[b0 + b][p][5], w2 = CF.k[b0 + b][p][6], w3 = CF.k[b0 + b][p][7];
-        T e00 = r[0][0] * inv; e00 = fma(ax, c[0][0][q0 + q], e00); e00 = fma(ay, yin[0][q], e00); e00 = fma(az, z0.v[q], e00);
-        T e10 = r[1][0] * inv; e10 = fma(ax, c[1][0][q0 + q], e10); e10 = fma(az, z1.v[q], e10); e10 = fma(ay, e00, e10);
-        T e01 = r[0][1] * inv; e01 = fma(ax, c[0][1][q0 + q], e01); e01 = fma(ay, yin[1][q], e01); e01 = fma(az, e00, e01);
-        T e11 = r[1][1] * inv; e11 = fma(ax, c[1][1][q0 + q], e11); e11 = fma(ay, e01, e11); e11 = fma(az, e10, e11);
-        c[0][0][q0 + q] = e00; c[1][0][q0 + q] = e10; c[0][1][q0 + q] = e01; c[1][1][q0 + q] = e11;
-        o0.v[q] = e01; o1.v[q] = e11;
-        m[0][0][0] = fma(w0, e00, m[0][0][0]); m[0][0][1] = fma(w1, e00, m[0][0][1]); m[0][0][2] = fma(w2, e00, m[0][0][2]); m[0][0][3] = fma(w3, e00, m[0][0][3]);
-        m[1][0][0] = fma(w0, e10, m[1][0][0]); m[1][0][1] = fma(w1, e10, m[1][0][1]); m[1][0][2] = fma(w2, e10, m[1][0][2]); m[1][0][3] = fma(w3, e10, m[1][0][3]);
-        m[0][1][0] = fma(w0, e01, m[0][1][0]); m[0][1][1] = fma(w1, e01, m[0][1][1]); m[0][1][2] = fma(w2, e01, m[0][1][2]); m[0][1][3] = fma(w3, e01, m[0][1][3]);
-        m[1][1][0] = fma(w0, e11, m[1][1][0]); m[1][1][1] = fma(w1, e11, m[1][1][1]); m[1][1][2] = fma(w2, e11, m[1][1][2]); m[1][1][3] = fma(w3, e11, m[1][1][3]);
+      for (int q = 0; q < NP; ++q) {
+        const int p = ch * CP + 2 * q;
+        const T(&kb)[8][BTE2_P] = CF.k[b0 + b];
+        const V2 inv = mk2(kb[0][p], kb[0][p + 1]), ax = mk2(kb[1][p], kb[1][p + 1]), ay = mk2(kb[2][p], kb[2][p + 1]),
+                 az = mk2(kb[3][p], kb[3][p + 1]);
+        const V2 w0 = mk2(kb[4][p], kb[4][p + 1]), w1 = mk2(kb[5][p], kb[5][p + 1]), w2 = mk2(kb[6][p], kb[6][p + 1]),
+                 w3 = mk2(kb[7][p], kb[7][p + 1]);
+        const V2 zq0 = mk2(z0.v[2 * q], z0.v[2 * q + 1]), zq1 = mk2(z1.v[2 * q], z1.v[2 * q + 1]);
+        V2 e00 = mul2(r[0][0], inv); e00 = fma2(ax, c[0][0][h0 + q], e00); e00 = fma2(ay, yin[0][q], e00); e00 = fma2(az, zq0, e00);
+        V2 e10 = mul2(r[1][0], inv); e10 = fma2(ax, c[1][0][h0 + q], e10); e10 = fma2(az, zq1, e10); e10 = fma2(ay, e00, e10);
+        V2 e01 = mul2(r[0][1], inv); e01 = fma2(ax, c[0][1][h0 + q], e01); e01 = fma2(ay, yin[1][q], e01); e01 = fma2(az, e00, e01);
+        V2 e11 = mul2(r[1][1], inv); e11 = fma2(ax, c[1][1][h0 + q], e11); e11 = fma2(ay, e01, e11); e11 = fma2(az, e10, e11);
+        c[0][0][h0 + q] = e00; c[1][0][h0 + q] = e10; c[0][1][h0 + q] = e01; c[1][1][h0 + q] = e11;
+        o0.v[2 * q] = e01.x; o0.v[2 * q + 1] = e01.y; o1.v[2 * q] = e11.x; o1.v[2 * q + 1] = e11.y;
+        acc2(m[0][0][0], w0, e00); acc2(m[0][0][1], w1, e00); acc2(m[0][0][2], w2, e00); acc2(m[0][0][3], w3, e00);
+        acc2(m[1][0][0], w0, e10); acc2(m[1][0][1], w1, e10); acc2(m[1][0][2], w2, e10); acc2(m[1][0][3], w3, e10);
+        acc2(m[0][1][0], w0, e01); acc2(m[0][1][1], w1, e01); acc2(m[0][1][2], w2, e01); acc2(m[0][1][3], w3, e01);
+        acc2(m[1][1][0], w0, e11); acc2(m[1][1][1], w1, e11); acc2(m[1][1][2], w2, e11); acc2(m[1][1][3], w3, e11);
       }
       zwr[cn * 32] = o0; zwr[(NC + cn) * 32] = o1;
     }
@@ -347,13 +367,13 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     if (t > 0) copy_out(t - 1);
     if (tid < 3 && mydep >= 0 && seen < t + 1 + D + mylag) peek = ld_acquire_gpu(P.prog + mydep);   // consumed by ensure() below
 
-    T m[2][2][4];
+    V2 m[2][2][4];                                     // moment partial sums of even / odd directions
 #pragma unroll
     for (int a = 0; a < 2; ++a)
 #pragma unroll
       for (int b = 0; b < 2; ++b)
 #pragma unroll
-        for (int q = 0; q < 4; ++q) m[a][b][q] = (T)0;
+        for (int q = 0; q < 4; ++q) m[a][b][q] = mk2((T)0, (T)0);
 
     Bte2Pair<T> in[2][2];
 #pragma unroll
@@ -366,11 +386,14 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     Ch *__restrict__ zwr = &S->zex[cur ^ 1][K][0][0][J];
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
-      T r[2][2];
+      V2 r[2][2];
 #pragma unroll
       for (int kk = 0; kk < 2; ++kk)
 #pragma unroll
-        for (int jj = 0; jj < 2; ++jj) r[jj][kk] = fma(bcx[b], in[jj][kk].x, bcy[b] * in[jj][kk].y);
+        for (int jj = 0; jj < 2; ++jj) {
+          const T rv = fma(bcx[b], in[jj][kk].x, bcy[b] * in[jj][kk].y);
+          r[jj][kk] = mk2(rv, rv);
+        }
       if (fast) {
 #pragma unroll
         for (int ch = 0; ch < NCH; ++ch) chunk(std::true_type{}, b, ch, r, m, rb, cur, true, zrd, zwr);
@@ -390,11 +413,11 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
             Bte2Mom<T> o;
             if (first) {
 #pragma unroll
-              for (int q = 0; q < 4; ++q) o.v[q] = m[jj][kk][q];
+              for (int q = 0; q < 4; ++q) o.v[q] = m[jj][kk][q].x + m[jj][kk][q].y;
             } else {
               const Bte2Mom<T> old = S->mold[cur][kk][jj][tid];
 #pragma unroll
-              for (int q = 0; q < 4; ++q) o.v[q] = old.v[q] + m[jj][kk][q];
+              for (int q = 0; q < 4; ++q) o.v[q] = old.v[q] + (m[jj][kk][q].x + m[jj][kk][q].y);
             }
             M[cbase[kk] + jj * 32 + (int64_t)t * 64] = o;
           }
@@ -409,7 +432,10 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
             for (int ch = 0; ch < NCH; ++ch) {
               Ch o;
 #pragma unroll
-              for (int q = 0; q < CP; ++q) o.v[q] = c[1][kk][b * BTE2_P + ch * CP + q];
+              for (int q = 0; q < CP; q += 2) {
+                const V2 v = c[1][kk][(b * BTE2_P + ch * CP + q) / 2];
+                o.v[q] = v.x; o.v[q + 1] = v.y;
+              }
               S->yst[cur ^ 1][K][kk * NC + b * NCH + ch] = o;
             }
       }
@@ -436,7 +462,10 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
         for (int ch = 0; ch < NCH; ++ch) {
           Ch o;
 #pragma unroll
-          for (int q = 0; q < CP; ++q) o.v[q] = c[jj][kk][b * BTE2_P + ch * CP + q];
+          for (int q = 0; q < CP; q += 2) {
+            const V2 v = c[jj][kk][(b * BTE2_P + ch * CP + q) / 2];
+            o.v[q] = v.x; o.v[q + 1] = v.y;
+          }
           xout[xpl2_index<T>(P, ty, tz, b0 + b, K, kk, jj, ch, J)] = o;
         }
   __threadfence();
