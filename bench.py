@@ -79,6 +79,16 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(sm)}
 
 
+def ncu_traffic(k, dtype):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch from the committed ncu --set full
+    capture (profiles/ncu_traffic.json, written from the .ncu-rep by hand; None if there is no capture)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            return json.load(f).get(f"config{k}_{dtype}", {}).get("dram_bytes_per_sweep_launch")
+    except OSError:
+        return None
+
+
 def oracle_sample(W, k, budget_s, steps):
     """Pick the largest replica of config k (same physical size, coarser grid) whose `steps` oracle
     iterations fit `budget_s` on this host; the oracle runs threaded over bands (bit-identical)."""
@@ -125,24 +135,55 @@ def run_reference(args, W):
     print(json.dumps(line), flush=True)
 
 
+class Ranks:
+    """Replicas-only multi-GPU plumbing (DESIGN.md section 8): one process per GPU, no data-path collective;
+    the only exchanges are a barrier and the MAX of a timing scalar.  Works with nccl (GPU) and gloo (CPU tests)."""
+
+    def __init__(self, backend="nccl", device=None):
+        import torch.distributed as dist
+        self.dist = dist
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        self.device = device
+        if self.world > 1 and not dist.is_initialized():
+            kw = {"device_id": device} if (backend == "nccl" and device is not None) else {}
+            dist.init_process_group(backend, **kw)
+
+    def barrier(self):
+        if self.world > 1:
+            self.dist.barrier()
+
+    def max(self, x):
+        import torch
+        t = torch.tensor([float(x)], dtype=torch.float64, device=self.device if self.device is not None else "cpu")
+        if self.world > 1:
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def aggregate(self, units_per_rank, seconds_local):
+        """whole-job throughput: all ranks' units / slowest rank's time"""
+        return self.world * units_per_rank / self.max(seconds_local)
+
+    def close(self):
+        if self.world > 1 and self.dist.is_initialized():
+            self.dist.destroy_process_group()
+
+
 def run_ours(args, W):
     import torch
-    import torch.distributed as dist
     import paper_2503_23657_b200 as bte
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+    R = Ranks("nccl", dev)
+    world, rank = R.world, R.rank
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        R.barrier()
         torch.cuda.synchronize()
 
     p = W.config(args.config)
@@ -164,10 +205,7 @@ def run_ours(args, W):
     e1.record()
     barrier()
     clocks = sampler.stop()
-    ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-    ms = float(ms.item())
+    ms = R.max(e0.elapsed_time(e1))
     sweep_ms, sweep_n = solver.sweep_timing()
     solver.set_sweep_timing(0)
     eps = solver.residual()
@@ -183,10 +221,7 @@ def run_ours(args, W):
     for _ in range(K):
         solver.solve_host(Qh, 1, reset=False, out=(dTh, None))
     barrier()
-    e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
-    e2e_s = float(e2e_s.item())
+    e2e_s = R.max(time.perf_counter() - t0)
 
     conv = None
     if args.converge and rank == 0:
@@ -220,8 +255,9 @@ def run_ours(args, W):
                         "d2h_bytes_per_step": dTh.numel() * 8,
                         "what": "bte_solve_host(Q pinned host -> 1 iteration -> dT pinned host) per step"},
                 "gpu_launches": solver.launches_per_iteration * K,
-                "roofline": {"bound": "alu", "kernel": "bte_sweep_kernel", "achieved": achieved, "peak": peak,
-                             "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                "roofline": {"bound": "alu", "kernel": "bte2_sweep_kernel" if solver.kernel_path == 2 else "bte_sweep_kernel",
+                             "achieved": achieved, "peak": peak,
+                             "unit": "TFLOP/s", "frac": achieved / peak, "traffic": ncu_traffic(args.config, dtype),
                              "peak_source": "derived: 148 SMs x %d FMA/clk x 2 x 1.965 GHz (DESIGN.md)" % (128 if dtype == "f32" else 64),
                              "ms_per_launch": sweep_avg_ms, "launches_timed": sweep_n,
                              "share_of_step": sweep_ms / ms if ms > 0 else None,
@@ -232,8 +268,7 @@ def run_ours(args, W):
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = time_oracle(W, args.config, budget_s=20.0, steps=1)[0]
         print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    R.close()
 
 
 def main():
