@@ -131,8 +131,12 @@ template <typename T> __device__ __forceinline__ Bte2Chunk<T> ldcg_chunk(const B
   memcpy(&r, &v, 16);
   return r;
 }
-// packed pairs of directions: fp32 uses the sm_100 two-wide FMA (FFMA2: two FMAs per issue slot, so the
-// non-FMA instructions of the step issue in the shadow of the FMA pipe); fp64 is two scalar DFMAs
+// packed pairs of directions: fp32 uses the sm_100 two-wide FMA (FFMA2: two FMAs per issue slot, which frees
+// issue slots for the non-FMA instructions of the step); fp64 is two scalar DFMAs.
+// Measured on B200 (_work microbenchmarks): FFMA2 whose coefficient operand is a PAIR of
+// uniform registers runs at half the FMA rate (64 FMA/clk/SM); with a broadcast scalar uniform register or
+// vector-register operands it runs at full rate, but those forms cost pair-assembly moves or 16 more registers
+// here (both tried, both slower in this kernel).
 template <typename T> struct Bte2V2;
 template <> struct Bte2V2<float> { typedef float2 t; };
 template <> struct Bte2V2<double> { typedef double2 t; };
