@@ -299,6 +299,9 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
     d.nty = (p->ny + 63) / 64; d.ntz = (p->nz + 2 * W - 1) / (2 * W); d.NU = p->nx + 31;
     d.nsteps = p->nx + 31 + W - 1;
     if (const char *e = std::getenv("BTE_V2_DBG")) d.dbg = std::atoi(e);
+    d.pub_mask = BTE2_PUB - 1; d.slack = BTE2_SLACK;
+    if (const char *e = std::getenv("BTE_V2_PUB")) { const int v = std::atoi(e); if (v == 4 || v == 8 || v == 16 || v == 32) d.pub_mask = v - 1; }
+    if (const char *e = std::getenv("BTE_V2_SLACK")) { const int v = std::atoi(e); if (v >= 0 && v <= 256) d.slack = v; }
     d.NS = (int64_t)p->nz * d.nty * d.NU * 64;
     d.ncell = N; d.inv_sumCtau = dv.inv_sumCtau;
     const int NBmax = dv.fp32 ? 2 : 1, G = (B + NBmax - 1) / NBmax;
@@ -434,7 +437,7 @@ void order_units2(Plan &pl, int slots) {
     const int lag[3] = {33, W + 1, 1};
     double a = 0;
     for (int k = 0; k < 3; ++k)
-      if (deps[k] >= 0) a = std::max(a, start[deps[k]] + (lag[k] + BTE2_DIST + BTE2_SLACK + BTE2_PUB) * steptime[deps[k]]);
+      if (deps[k] >= 0) a = std::max(a, start[deps[k]] + (lag[k] + BTE2_DIST + pl.d2.slack + pl.d2.pub_mask + 1) * steptime[deps[k]]);
     return a;
   };
   typedef std::pair<double, int> Key;

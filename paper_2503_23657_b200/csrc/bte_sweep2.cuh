@@ -30,7 +30,7 @@
 #define BTE2_MAXB 16      // bands in the parameter table
 #define BTE2_PUB 8        // progress is published every PUB steps
 #define BTE2_DIST 2       // cp.async prefetch distance in steps
-#define BTE2_SLACK 24     // extra steps a unit lets the units it follows get ahead before it starts
+#define BTE2_SLACK 0      // extra steps a unit lets the units it follows get ahead before it starts
 #define BTE2_TYROWS 64    // tile rows along y' (32 lanes x 2)
 
 template <typename T> struct alignas(16) Bte2Coefs {   // kernel parameter (constant bank 0)
@@ -70,7 +70,8 @@ struct Bte2Dev {
   void *Gf;                         // T diffuse inflow [f][b][tb][ta]
   int64_t gf_off[6];
   double *dT, *q, *qmag, *red;      // fp64 outputs in physical layout; residual partials
-  int32_t n_red_blocks, pad1;
+  int32_t n_red_blocks, pub_mask;   // progress is published when (t & pub_mask) == pub_mask
+  int32_t slack, pad1;
   int64_t ncell;
   double inv_sumCtau;
 };
@@ -298,7 +299,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
           for (int q = 0; q < CP; q += 2) c[jj][kk][(b * BTE2_P + ch * CP + q) / 2] = mk2(v.v[q], v.v[q + 1]);
         }
 
-  ensure(D + BTE2_SLACK);
+  ensure(D + P.slack);
   __syncthreads();
 #pragma unroll
   for (int t1 = 0; t1 < D; ++t1) {
@@ -447,7 +448,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     cp_async_wait<D - 1>();            // everything step t+1 reads has landed
     if (tid < 3) ensure(t + 1 + D);    // ... and what step t+1 prefetches has been published upstream
     __syncthreads();
-    if ((t & (BTE2_PUB - 1)) == BTE2_PUB - 1 && tid == 0) {   // faces and moments of steps < t are in global memory
+    if ((t & P.pub_mask) == P.pub_mask && tid == 0) {   // faces and moments of steps < t are in global memory
       __threadfence();
       st_release_gpu(P.prog + unit, ebase + t);
     }
