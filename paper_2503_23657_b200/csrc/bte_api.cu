@@ -51,7 +51,7 @@ struct Plan {
   Bte2Coefs<float> cf32{};
   Bte2Coefs<double> cf64{};
   size_t smem2 = 0;
-  size_t x2_chunks = 0, y2_chunks = 0, z2_chunks = 0;
+  size_t x2_chunks = 0, y2_chunks = 0, z2_chunks = 0, y2_slot = 0, z2_slot = 0;
   size_t xpl_elems[8]{}, ypl_elems[8]{}, zpl_elems[8]{};
 };
 
@@ -338,8 +338,10 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
     d.n_units = (int32_t)pl.units2.size();
     const size_t nch = BTE2_P * tsz / 16;
     pl.x2_chunks = (size_t)d.ntz * d.nty * B * W * 2 * 2 * nch * 32;
-    pl.y2_chunks = (size_t)(d.nty + 1) * d.ntz * B * W * d.nx * 2 * nch;
-    pl.z2_chunks = (size_t)(d.ntz + 1) * d.nty * B * d.NU * 2 * nch * 32;
+    pl.y2_slot = (size_t)d.ntz * B * W * d.nx * 2 * nch;
+    pl.z2_slot = (size_t)d.nty * B * d.NU * 2 * nch * 32;
+    pl.y2_chunks = (size_t)(d.nty + 2) * pl.y2_slot;
+    pl.z2_chunks = (size_t)(d.ntz + 2) * pl.z2_slot;
     int64_t off = 0;
     for (int f = 0; f < 6; ++f) {
       const int a = f >> 1;
@@ -380,7 +382,7 @@ size_t bind(Plan &pl, unsigned char *ws) {
     d.Gf = take(std::max<size_t>(pl.gf_elems, 1) * tsz);
     for (int o = 0; o < 8; ++o) {
       d.oct[o].M = take(NS2 * 4 * tsz);
-      d.oct[o].xin = take(pl.x2_chunks * 16); d.oct[o].xout = take(pl.x2_chunks * 16);
+      d.oct[o].xin = take(pl.x2_chunks * 16); d.oct[o].xout = take(2 * pl.x2_chunks * 16);
       d.oct[o].ypl = take(pl.y2_chunks * 16); d.oct[o].zpl = take(pl.z2_chunks * 16);
     }
     pl.state_end = off;
@@ -525,6 +527,26 @@ bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t
     const int ep = (int)(h->iters % 30000) + 1;
     if (ep == 1 && h->iters > 0) CK(cudaMemsetAsync(d.prog, 0, (size_t)d.n_units * 4, st));
     d.epoch = ep;
+    {   // inflow sources / outflow buffers of this iteration (parity of the epoch)
+      const size_t cur = (size_t)(ep & 1), prev = cur ^ 1;
+      auto xo = [&](int o, size_t par) { return (char *)d.oct[o].xout + par * pl.x2_chunks * 16; };
+      auto yo = [&](int o, size_t par) { return (char *)d.oct[o].ypl + ((size_t)d.nty + par) * pl.y2_slot * 16; };
+      auto zo = [&](int o, size_t par) { return (char *)d.oct[o].zpl + ((size_t)d.ntz + par) * pl.z2_slot * 16; };
+      for (int o = 0; o < 8; ++o) {
+        Bte2Oct &O = d.oct[o];
+        O.xdst = xo(o, cur); O.ydstN = yo(o, cur); O.zdstN = zo(o, cur);
+        O.xprev = xo(o, prev); O.yprev = yo(o, prev); O.zprev = zo(o, prev);
+        const int sg[3] = {O.sx, O.sy, O.sz};
+        const void *ghost[3] = {O.xin, O.ypl, O.zpl};
+        const void *src[3];
+        for (int a = 0; a < 3; ++a) {
+          const int type = d.face_type[2 * a + (sg[a] > 0 ? 0 : 1)];
+          const int from = type == 2 ? (o ^ (1 << a)) : o;
+          src[a] = type < 2 ? ghost[a] : (a == 0 ? (const void *)xo(from, prev) : (a == 1 ? (const void *)yo(from, prev) : (const void *)zo(from, prev)));
+        }
+        O.xsrc = src[0]; O.ysrc0 = src[1]; O.zsrc0 = src[2];
+      }
+    }
     if (pl.any_diffuse_face) bte2_gdiff_kernel<T><<<bgrid, 256, 0, st>>>(d);
     bte2_ghost_kernel<T><<<bgrid, 256, 0, st>>>(d);
     const bool tm = h->timing && h->ev_used + 2 <= h->ev.size();

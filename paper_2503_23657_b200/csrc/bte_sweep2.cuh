@@ -48,8 +48,16 @@ struct Bte2Unit {
 struct Bte2Oct {
   int32_t sx, sy, sz, cls;
   void *M;                  // T [NS][4]   moment accumulator of this octant (skewed class layout)
-  void *xin, *xout;         // x face planes
-  void *ypl, *zpl;          // y / z face planes, slots 0..nty / 0..ntz
+  void *xin, *xout;         // x face planes: inflow ghost plane; outflow, two buffers (iteration parity)
+  void *ypl, *zpl;          // y / z face planes: slot 0 = inflow ghost plane, slots 1..n-1 = hand-off between tiles,
+                            // slots n, n+1 = outflow of the last tile row (lagged boundary store), two buffers
+  // set by the host for every iteration (epoch parity): where this octant's sweep reads its box-face inflow
+  // (its ghost plane for isothermal / diffuse faces; for specular / periodic faces directly the outflow buffer
+  // the mirrored / same octant wrote in the PREVIOUS iteration -- same layout, so no copy is needed) and which
+  // outflow buffers it writes (dst) / the boundary kernels read (prev)
+  const void *xsrc, *ysrc0, *zsrc0;
+  void *xdst, *ydstN, *zdstN;
+  const void *xprev, *yprev, *zprev;
 };
 
 struct Bte2Dev {
@@ -188,8 +196,8 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
   const bool first = un.dep_prev < 0;                  // first band group of this octant: M is written, not added to
   const int ebase = P.epoch << 16;
 
-  const Ch *xin = reinterpret_cast<const Ch *>(O.xin);
-  Ch *xout = reinterpret_cast<Ch *>(O.xout);
+  const Ch *xin = reinterpret_cast<const Ch *>(O.xsrc);
+  Ch *xout = reinterpret_cast<Ch *>(O.xdst);
   Bte2Mom<T> *M = reinterpret_cast<Bte2Mom<T> *>(O.M);
   const Bte2Pair<T> *dTQ = reinterpret_cast<const Bte2Pair<T> *>(P.dTQ[O.cls]);
 
@@ -202,13 +210,17 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
   }
   // plane pointers of this thread at step 0; all advance by a constant stride per step
   //   z inflow staging: element e = tid + q*NT of the [b][jj][ch][lane] block of step u
-  const Ch *zsrc = reinterpret_cast<const Ch *>(O.zpl) + zpl2_index<T>(P, tz, ty, b0, 0, 0, 0, 0);
+  const Ch *zsrc = (tz == 0 ? reinterpret_cast<const Ch *>(O.zsrc0) : reinterpret_cast<const Ch *>(O.zpl) + zpl2_index<T>(P, tz, 0, 0, 0, 0, 0, 0)) +
+                   zpl2_index<T>(P, 0, ty, b0, 0, 0, 0, 0);
   const int64_t zstep = 2 * NCH * 32, zband = (int64_t)P.NU * 2 * NCH * 32;
-  Ch *zdst = reinterpret_cast<Ch *>(O.zpl) + zpl2_index<T>(P, tz + 1, ty, b0, 0, 0, 0, 0);
+  Ch *zdst = (tz == P.ntz - 1 ? reinterpret_cast<Ch *>(O.zdstN) : reinterpret_cast<Ch *>(O.zpl) + zpl2_index<T>(P, tz + 1, 0, 0, 0, 0, 0, 0)) +
+             zpl2_index<T>(P, 0, ty, b0, 0, 0, 0, 0);
   //   y planes: lane l < 2*NC of warp K loads chunk (b, kk, ch) of the cell i' = t - K
   const int yb = J / (2 * NCH), ykk = (J / NCH) & 1, ych = J % NCH;
-  const Ch *ysrc = reinterpret_cast<const Ch *>(O.ypl) + ypl2_index<T>(P, ty, tz, b0 + (J < 2 * NC ? yb : 0), K, 0, ykk, ych) - (int64_t)K * 2 * NCH;
-  Ch *ydst = reinterpret_cast<Ch *>(O.ypl) + ypl2_index<T>(P, ty + 1, tz, b0 + (J < 2 * NC ? yb : 0), K, 0, ykk, ych);
+  const Ch *ysrc = (ty == 0 ? reinterpret_cast<const Ch *>(O.ysrc0) : reinterpret_cast<const Ch *>(O.ypl) + ypl2_index<T>(P, ty, 0, 0, 0, 0, 0, 0)) +
+                   ypl2_index<T>(P, 0, tz, b0 + (J < 2 * NC ? yb : 0), K, 0, ykk, ych) - (int64_t)K * 2 * NCH;
+  Ch *ydst = (ty == P.nty - 1 ? reinterpret_cast<Ch *>(O.ydstN) : reinterpret_cast<Ch *>(O.ypl) + ypl2_index<T>(P, ty + 1, 0, 0, 0, 0, 0, 0)) +
+             ypl2_index<T>(P, 0, tz, b0 + (J < 2 * NC ? yb : 0), K, 0, ykk, ych);
 
   // ---- progress of the units this one follows: lanes 0..2 of warp 0 keep the last value seen in a register
   const int mydep = tid == 0 ? un.dep_y : (tid == 1 ? un.dep_z : (tid == 2 ? un.dep_prev : -1));
@@ -505,14 +517,14 @@ __device__ __forceinline__ Bte2Chunk<T> *bte2_plane_chunk(const Bte2Dev &P, int 
   const Bte2Oct &O = P.oct[o];
   if (a == 0) {
     const int ty = jp >> 6, J = (jp & 63) >> 1, jj = jp & 1, tz = kp / (2 * P.W), K = (kp % (2 * P.W)) >> 1, kk = kp & 1;
-    return reinterpret_cast<Bte2Chunk<T> *>(side ? O.xout : O.xin) + xpl2_index<T>(P, ty, tz, b, K, kk, jj, ch, J);
+    return reinterpret_cast<Bte2Chunk<T> *>(side ? const_cast<void *>(O.xprev) : O.xin) + xpl2_index<T>(P, ty, tz, b, K, kk, jj, ch, J);
   }
   if (a == 1) {
     const int tz = kp / (2 * P.W), K = (kp % (2 * P.W)) >> 1, kk = kp & 1;
-    return reinterpret_cast<Bte2Chunk<T> *>(O.ypl) + ypl2_index<T>(P, side ? P.nty : 0, tz, b, K, ip, kk, ch);
+    return reinterpret_cast<Bte2Chunk<T> *>(side ? const_cast<void *>(O.yprev) : O.ypl) + ypl2_index<T>(P, 0, tz, b, K, ip, kk, ch);
   }
   const int ty = jp >> 6, J = (jp & 63) >> 1, jj = jp & 1;
-  return reinterpret_cast<Bte2Chunk<T> *>(O.zpl) + zpl2_index<T>(P, side ? P.ntz : 0, ty, b, ip + J, jj, ch, J);
+  return reinterpret_cast<Bte2Chunk<T> *>(side ? const_cast<void *>(O.zprev) : O.zpl) + zpl2_index<T>(P, 0, ty, b, ip + J, jj, ch, J);
 }
 
 struct Bte2Face { int na, nb; };
@@ -561,7 +573,8 @@ __global__ void bte2_gdiff_kernel(const __grid_constant__ Bte2Dev P) {
   }
 }
 
-// Fill the inflow plane of every octant on every axis from the lagged outflow (Eq. 5-7 + periodic).
+// Fill the inflow ghost planes of isothermal (Eq. 5) and diffuse (Eq. 6) box faces.  Specular (Eq. 7) and periodic
+// faces need none: their inflow IS another outflow plane of the previous iteration (Bte2Oct::xsrc / ysrc0 / zsrc0).
 template <typename T>
 __global__ void bte2_ghost_kernel(const __grid_constant__ Bte2Dev P) {
   constexpr int CP = 16 / sizeof(T), NCH = BTE2_P / CP;
@@ -573,6 +586,7 @@ __global__ void bte2_ghost_kernel(const __grid_constant__ Bte2Dev P) {
       const int sg = a == 0 ? O.sx : (a == 1 ? O.sy : O.sz);
       const int side = sg > 0 ? 0 : 1, f = 2 * a + side;   // physical face the octant enters through
       const int type = P.face_type[f];
+      if (type >= 2) continue;      // specular / periodic: the sweep reads the lagged outflow buffer directly
       const Bte2Face g = bte2_face(P, a);
       const int64_t n = (int64_t)g.na * g.nb * P.B * NCH;
       for (int64_t e = gtid; e < n; e += gstride) {
@@ -589,14 +603,6 @@ __global__ void bte2_ghost_kernel(const __grid_constant__ Bte2Dev P) {
           const T gv = Gf[P.gf_off[f] + ((int64_t)b * g.nb + tb) * g.na + ta];
 #pragma unroll
           for (int q = 0; q < CP; ++q) v.v[q] = gv;
-        } else if (type == 2) {   // specular: mirrored octant leaves through this face at the same cell
-          int ip2, jp2, kp2;
-          bte2_face_cell(P, o ^ (1 << a), a, side, ta, tb, ip2, jp2, kp2);
-          v = ldcg_chunk<T>(bte2_plane_chunk<T>(P, o ^ (1 << a), a, 1, b, ch, ip2, jp2, kp2));
-        } else {                  // periodic: same octant leaves through the opposite face
-          int ip2, jp2, kp2;
-          bte2_face_cell(P, o, a, side ^ 1, ta, tb, ip2, jp2, kp2);
-          v = ldcg_chunk<T>(bte2_plane_chunk<T>(P, o, a, 1, b, ch, ip2, jp2, kp2));
         }
         *bte2_plane_chunk<T>(P, o, a, 0, b, ch, ip, jp, kp) = v;
       }
