@@ -276,7 +276,7 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
     pl.ypl_elems[o] = dv.has_y ? (size_t)(dv.nty + 1) * O.nitems * dv.nz * dv.nx * BTE_P : 0;
     pl.zpl_elems[o] = dv.has_z ? (size_t)(dv.ntz + 1) * O.nitems * dv.nty * dv.NU * BTE_P * 32 : 0;
   }
-  dv.n_red_blocks = (int)std::min<int64_t>((N + 255) / 256, 148 * 8);
+  dv.n_red_blocks = (int)std::min<int64_t>((N + 255) / 256, 148 * 16);
 
   // ---- fast path: 3-D, all solid, 16 directions in each of the 8 octants with identical |s|, w tables
   // (mirror-symmetric quadrature), <= 16 bands.  Anything else runs the generic kernels above.
@@ -527,6 +527,7 @@ bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t
     const int ep = (int)(h->iters % 30000) + 1;
     if (ep == 1 && h->iters > 0) CK(cudaMemsetAsync(d.prog, 0, (size_t)d.n_units * 4, st));
     d.epoch = ep;
+    d.fill_iso = h->iters == 0;
     {   // inflow sources / outflow buffers of this iteration (parity of the epoch)
       const size_t cur = (size_t)(ep & 1), prev = cur ^ 1;
       auto xo = [&](int o, size_t par) { return (char *)d.oct[o].xout + par * pl.x2_chunks * 16; };

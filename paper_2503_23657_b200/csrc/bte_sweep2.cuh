@@ -79,7 +79,7 @@ struct Bte2Dev {
   int64_t gf_off[6];
   double *dT, *q, *qmag, *red;      // fp64 outputs in physical layout; residual partials
   int32_t n_red_blocks, pub_mask;   // progress is published when (t & pub_mask) == pub_mask
-  int32_t slack, pad1;
+  int32_t slack, fill_iso;          // fill_iso: (re)write the constant isothermal ghost planes (first iteration only)
   int64_t ncell;
   double inv_sumCtau;
 };
@@ -587,11 +587,16 @@ __global__ void bte2_ghost_kernel(const __grid_constant__ Bte2Dev P) {
       const int side = sg > 0 ? 0 : 1, f = 2 * a + side;   // physical face the octant enters through
       const int type = P.face_type[f];
       if (type >= 2) continue;      // specular / periodic: the sweep reads the lagged outflow buffer directly
+      if (type == 0 && !P.fill_iso) continue;   // isothermal planes are constant: written once
       const Bte2Face g = bte2_face(P, a);
       const int64_t n = (int64_t)g.na * g.nb * P.B * NCH;
       for (int64_t e = gtid; e < n; e += gstride) {
-        // ta fastest, then chunk, so that neighbouring threads touch neighbouring lanes of a plane
-        const int ta = (int)(e % g.na), ch = (int)((e / g.na) % NCH), tb = (int)((e / ((int64_t)g.na * NCH)) % g.nb);
+        // thread order follows the plane layouts so that writes coalesce: x planes [..][chunk][J]: j fastest;
+        // y planes [..][i'][kk][chunk]: chunk, then i; z planes [..][u][jj][chunk][J]: j fastest, then chunk, then i
+        int ta, tb, ch;
+        if (a == 0) { ta = (int)(e % g.na); ch = (int)((e / g.na) % NCH); tb = (int)((e / ((int64_t)g.na * NCH)) % g.nb); }
+        else if (a == 1) { ch = (int)(e % NCH); ta = (int)((e / NCH) % g.na); tb = (int)((e / ((int64_t)g.na * NCH)) % g.nb); }
+        else { tb = (int)(e % g.nb); ch = (int)((e / g.nb) % NCH); ta = (int)((e / ((int64_t)g.nb * NCH)) % g.na); }
         const int b = (int)(e / ((int64_t)g.na * NCH * g.nb));
         int ip, jp, kp;
         bte2_face_cell(P, o, a, side, ta, tb, ip, jp, kp);
@@ -615,7 +620,7 @@ __global__ void bte2_ghost_kernel(const __grid_constant__ Bte2Dev P) {
 // dT^{n+1} = M0 / sum(C/tau) (Eq. 16), q = M1 (Eq. 4), residual partial sums (Eq. 23); octant partials are
 // summed in fp64 in a fixed order; dT is written back into the four skewed class copies the sweep reads.
 template <typename T>
-__global__ void __launch_bounds__(256) bte2_update_kernel(const __grid_constant__ Bte2Dev P) {
+__global__ void __launch_bounds__(256, 4) bte2_update_kernel(const __grid_constant__ Bte2Dev P) {
   double sT = 0, mT = 0, sq = 0, mq = 0;
   for (int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; c < P.ncell; c += (int64_t)gridDim.x * blockDim.x) {
     const int i = (int)(c % P.nx), j = (int)((c / P.nx) % P.ny), k = (int)(c / ((int64_t)P.nx * P.ny));
