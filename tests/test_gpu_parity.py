@@ -250,3 +250,13 @@ def test_config4_full_sampled(bte):
     p = W.config(4)
     out = check(bte, p, 2, checkpoints=(1,))
     assert out[-1][1] <= 1e-4
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("prec", [W.FP64, W.FP32_STORE_FP64_ACC])
+def test_config4_replica_converged_state(bte, prec):
+    """Like-for-like converged-state check: a 32x16x16 replica of the large slab is
+    iterated far towards its fixed point on both sides; rounding differences must not accumulate."""
+    p = W.config(4, grid=(32, 16, 16))
+    out = check(bte, p, 400, precision=prec, checkpoints=(100,))
+    assert out[-1][3][0] < 1e-5          # oracle eps_T: well converged
