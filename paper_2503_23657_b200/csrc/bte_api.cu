@@ -439,7 +439,7 @@ void order_units2(Plan &pl, int slots) {
     const int lag[3] = {33, W + 1, 1};
     double a = 0;
     for (int k = 0; k < 3; ++k)
-      if (deps[k] >= 0) a = std::max(a, start[deps[k]] + (lag[k] + BTE2_DIST + pl.d2.slack + pl.d2.pub_mask + 1) * steptime[deps[k]]);
+      if (deps[k] >= 0) a = std::max(a, start[deps[k]] + (lag[k] + BTE2_DIST(W) + pl.d2.slack + pl.d2.pub_mask + 1) * steptime[deps[k]]);
     return a;
   };
   typedef std::pair<double, int> Key;
@@ -565,7 +565,7 @@ bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t
 template <typename T, int W>
 bte_status setup_sweep2_W(bte_solver *h) {
   Plan &pl = h->pl;
-  pl.smem2 = sizeof(Bte2Smem<T, sizeof(T) == 4 ? 2 : 1, W, BTE2_DIST>);
+  pl.smem2 = sizeof(Bte2Smem<T, sizeof(T) == 4 ? 2 : 1, W, BTE2_DIST(W)>);
   CK(cudaFuncSetAttribute(bte2_sweep_kernel<T, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem2));
   int occ = 0;
   CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bte2_sweep_kernel<T, W>, W * 32, pl.smem2));

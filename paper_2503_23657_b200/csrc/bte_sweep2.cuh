@@ -29,7 +29,7 @@
 #define BTE2_P 16         // directions per octant
 #define BTE2_MAXB 16      // bands in the parameter table
 #define BTE2_PUB 8        // progress is published every PUB steps
-#define BTE2_DIST 2       // cp.async prefetch distance in steps
+#define BTE2_DIST(W) ((W) >= 8 ? 2 : 1)   // cp.async prefetch distance in steps (1 lets two 4-warp CTAs share an SM)
 #define BTE2_SLACK 0      // extra steps a unit lets the units it follows get ahead before it starts
 #define BTE2_TYROWS 64    // tile rows along y' (32 lanes x 2)
 
@@ -494,7 +494,7 @@ template <typename T, int W>
 __global__ void __launch_bounds__(W * 32) bte2_sweep_kernel(const __grid_constant__ Bte2Dev P,
                                                             const __grid_constant__ Bte2Coefs<T> CF) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  constexpr int NBMAX = sizeof(T) == 4 ? 2 : 1, D = BTE2_DIST;
+  constexpr int NBMAX = sizeof(T) == 4 ? 2 : 1, D = BTE2_DIST(W);
   __shared__ int s_unit;
   for (;;) {
     __syncthreads();
