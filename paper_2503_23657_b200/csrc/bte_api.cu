@@ -45,7 +45,8 @@ struct Plan {
   bool any_diffuse_face = false;
   size_t gf_elems = 0;
   // fast path (bte_sweep2.cuh)
-  bool v2 = false;
+  bool v2 = false, masked2 = false;
+  std::vector<uint32_t> codeP[4];
   Bte2Dev d2{};
   std::vector<Bte2Unit> units2;
   Bte2Coefs<float> cf32{};
@@ -280,7 +281,8 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
 
   // ---- fast path: 3-D, all solid, 16 directions in each of the 8 octants with identical |s|, w tables
   // (mirror-symmetric quadrature), <= 16 bands.  Anything else runs the generic kernels above.
-  bool v2 = p->dim == 3 && nif == 0 && nsolid == N && B <= BTE2_MAXB && p->nx <= 60000 && p->ny % 2 == 0 && p->nz % 2 == 0;
+  bool v2 = p->dim == 3 && B <= BTE2_MAXB && p->nx <= 60000 && p->ny % 2 == 0 && p->nz % 2 == 0;
+  pl.masked2 = nsolid != N;
   if (const char *e = std::getenv("BTE_FORCE_GENERIC")) if (e[0] == '1') v2 = false;
   for (int o = 0; o < 8 && v2; ++o) {
     if ((int)od[o].size() != BTE2_P) v2 = false;
@@ -335,6 +337,21 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
       U.dep_prev = g > 0 ? uid(g - 1, ty, tz, o) : -1;
       U.b0 = g * NBmax; U.nb = std::min(NBmax, B - U.b0);
     }
+    d.n_iface = nif; d.iface_type = p->interface_bc.type;
+    for (int b = 0; b < B; ++b) d.iface_e0[b] = pl.band[b] * p->interface_bc.dT_wall;
+    if (pl.masked2) {
+      const size_t NPp = (size_t)(p->nz / 2) * d.nty * d.NU * 32;
+      for (int cl = 0; cl < 4; ++cl) {
+        pl.codeP[cl].assign(NPp, 0u);
+        for (int k = 0; k < p->nz; ++k) for (int j = 0; j < p->ny; ++j) for (int i = 0; i < p->nx; ++i) {
+          const int ipc = (cl & 1) ? p->nx - 1 - i : i, jpc = (cl & 2) ? p->ny - 1 - j : j;
+          const int ty = jpc >> 6, J = (jpc & 63) >> 1;
+          const size_t idx = (((size_t)(k >> 1) * d.nty + ty) * d.NU + (ipc + J)) * 32 + J;
+          const uint32_t byte = pl.code[(size_t)i + (size_t)p->nx * (j + (size_t)p->ny * k)];
+          pl.codeP[cl][idx] |= byte << (8 * ((j & 1) + 2 * (k & 1)));
+        }
+      }
+    }
     d.n_units = (int32_t)pl.units2.size();
     const size_t nch = BTE2_P * tsz / 16;
     pl.x2_chunks = (size_t)d.ntz * d.nty * B * W * 2 * 2 * nch * 32;
@@ -372,7 +389,18 @@ size_t bind(Plan &pl, unsigned char *ws) {
     Bte2Dev &d = pl.d2;
     const size_t NS2 = (size_t)d.NS;
     d.units = (const Bte2Unit *)take(pl.units2.size() * sizeof(Bte2Unit));
+    if (pl.masked2) {
+      d.code = dv.code;
+      for (int c = 0; c < 4; ++c) d.codeP[c] = (const uint32_t *)take((size_t)(dv.nz / 2) * d.nty * d.NU * 32 * 4);
+      d.iface = d.n_iface ? (const int32_t *)take((size_t)6 * N * 4) : nullptr;
+      d.iface_info = d.n_iface ? (const int32_t *)take((size_t)d.n_iface * 4) : nullptr;
+    } else {
+      d.code = nullptr; d.iface = nullptr; d.iface_info = nullptr;
+      for (int c = 0; c < 4; ++c) d.codeP[c] = nullptr;
+    }
     pl.state_begin = off;
+    d.Gi = d.n_iface ? take((size_t)d.n_iface * d.B * tsz) : nullptr;
+    d.Hpart = d.n_iface ? (double *)take((size_t)d.n_iface * d.B * 4 * 8) : nullptr;
     d.prog = (int32_t *)take((size_t)d.n_units * 4);
     d.ticket = (int32_t *)take(256);
     dv.red = (double *)take((size_t)(4 * dv.n_red_blocks + 4) * 8);
@@ -515,7 +543,8 @@ bte_status skew(bte_solver *h, const double *src, double scale, int which, cudaS
 
 template <typename T, int W>
 void launch_sweep2(bte_solver *h, const Bte2Coefs<T> &cf, cudaStream_t st) {
-  bte2_sweep_kernel<T, W><<<h->sweep_grid, W * 32, h->pl.smem2, st>>>(h->pl.d2, cf);
+  if (h->pl.masked2) bte2_sweep_kernel<T, W, true><<<h->sweep_grid, W * 32, h->pl.smem2, st>>>(h->pl.d2, cf);
+  else bte2_sweep_kernel<T, W, false><<<h->sweep_grid, W * 32, h->pl.smem2, st>>>(h->pl.d2, cf);
 }
 
 template <typename T>
@@ -566,9 +595,14 @@ template <typename T, int W>
 bte_status setup_sweep2_W(bte_solver *h) {
   Plan &pl = h->pl;
   pl.smem2 = sizeof(Bte2Smem<T, sizeof(T) == 4 ? 2 : 1, W, BTE2_DIST(W)>);
-  CK(cudaFuncSetAttribute(bte2_sweep_kernel<T, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem2));
   int occ = 0;
-  CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bte2_sweep_kernel<T, W>, W * 32, pl.smem2));
+  if (pl.masked2) {
+    CK(cudaFuncSetAttribute(bte2_sweep_kernel<T, W, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem2));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bte2_sweep_kernel<T, W, true>, W * 32, pl.smem2));
+  } else {
+    CK(cudaFuncSetAttribute(bte2_sweep_kernel<T, W, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem2));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bte2_sweep_kernel<T, W, false>, W * 32, pl.smem2));
+  }
   if (occ < 1) { g_last_cuda = (int)cudaErrorLaunchOutOfResources; return BTE_ERR_CUDA; }
   h->sweep_grid = (int)std::min<int64_t>(pl.d2.n_units, (int64_t)h->num_sms * occ);
   pl.nthreads = W * 32;
@@ -649,6 +683,14 @@ bte_status bte_create(const bte_problem *p, void *d_workspace, size_t bytes, voi
   if (pl.v2) {
     order_units2(pl, h->sweep_grid);
     CKD(cudaMemcpyAsync((void *)pl.d2.units, pl.units2.data(), pl.units2.size() * sizeof(Bte2Unit), cudaMemcpyHostToDevice, s));
+    if (pl.masked2) {
+      for (int c = 0; c < 4; ++c)
+        CKD(cudaMemcpyAsync((void *)pl.d2.codeP[c], pl.codeP[c].data(), pl.codeP[c].size() * 4, cudaMemcpyHostToDevice, s));
+      if (pl.d2.n_iface) {
+        CKD(cudaMemcpyAsync((void *)pl.d2.iface, pl.iface.data(), pl.iface.size() * 4, cudaMemcpyHostToDevice, s));
+        CKD(cudaMemcpyAsync((void *)pl.d2.iface_info, pl.iface_info.data(), pl.iface_info.size() * 4, cudaMemcpyHostToDevice, s));
+      }
+    }
   } else {
     if (dv.n_iface) {
       CKD(cudaMemcpyAsync(dv.iface, pl.iface.data(), pl.iface.size() * 4, cudaMemcpyHostToDevice, s));

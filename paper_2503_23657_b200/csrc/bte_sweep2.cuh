@@ -82,6 +82,17 @@ struct Bte2Dev {
   int32_t slack, fill_iso;          // fill_iso: (re)write the constant isothermal ghost planes (first iteration only)
   int64_t ncell;
   double inv_sumCtau;
+  // voxel masks (all null / 0 when every cell is solid).  Cell byte: bit0 solid, bit 1+f: the neighbour across
+  // face f (x-,x+,y-,y+,z-,z+) is a solid/void interface (or a periodic wrap onto a void cell).
+  const uint8_t *code;              // [ncell] physical layout
+  const uint32_t *codeP[4];         // per x/y-flip class: the 4 cell bytes of a thread's 2x2 patch, byte (j&1) + 2 (k&1),
+                                    // index ((kz * nty + ty) * NU + (i' + J)) * 32 + J, kz = physical k / 2
+  const int32_t *iface;             // [6][ncell] interface-face id or -1
+  const int32_t *iface_info;        // [n_iface] face code f
+  void *Gi;                         // T [n_iface][B] interface inflow of this iteration (Eq. 5 / Eq. 6)
+  double *Hpart;                    // [n_iface][B][4] outgoing hemispherical partial sums per octant slot
+  int32_t n_iface, iface_type;
+  double iface_e0[BTE2_MAXB];       // isothermal interface inflow C_b dT_w / 4pi
 };
 
 // ------------------------------------------------------------------ layouts (host + device)
@@ -130,6 +141,7 @@ __device__ __forceinline__ void cp_async(void *smem_dst, const void *gsrc) {
   const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
   if (BYTES == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
   else if (BYTES == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+  else if (BYTES == 4) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
@@ -174,10 +186,11 @@ template <typename T, int NB, int W, int D> struct Bte2Smem {
   Ch yst[2][W][2 * NC];              // [parity][warp][kk*NC + chunk]: jj=1 rows of lane Jl, copied out one step later
   Bte2Mom<T> mold[2][2][2][W * 32];  // [parity][kk][jj][tid] previous content of the moment accumulator
   Bte2Pair<T> inp[D + 1][2][2][W * 32];    // [ring][kk][jj][tid] (dT, Q/sumC) of the cell
+  uint32_t codes[D + 1][W * 32];           // [ring][tid] cell bytes of the thread's patch (masked grids only)
 };
 
 // ------------------------------------------------------------------ one unit = (octant, band group, tile)
-template <typename T, int NB, int W, int D>
+template <typename T, int NB, int W, int D, bool MASKED>
 __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<T> &CF, const Bte2Unit &un,
                                               unsigned char *smem_raw, int unit) {
   typedef Bte2Smem<T, NB, W, D> SM;
@@ -207,6 +220,13 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
   for (int kk = 0; kk < 2; ++kk) {
     const int kp = kp0 + kk, k = vthread ? (O.sz > 0 ? kp : P.nz - 1 - kp) : 0;
     cbase[kk] = (((int64_t)k * P.nty + ty) * P.NU) * 64 + J - (int64_t)K * 64;
+  }
+  // voxel mask: patch-code stream of this thread, face indices of this octant
+  const int fu[3] = {O.sx > 0 ? 0 : 1, O.sy > 0 ? 2 : 3, O.sz > 0 ? 4 : 5};      // upwind faces x, y, z
+  const uint32_t *cpsrc = nullptr;
+  if (MASKED) {
+    const int kz = (vthread ? (O.sz > 0 ? kp0 : P.nz - 2 - kp0) : 0) >> 1;
+    cpsrc = P.codeP[O.cls] + (((int64_t)kz * P.nty + ty) * P.NU) * 32 + J - (int64_t)K * 32;
   }
   // plane pointers of this thread at step 0; all advance by a constant stride per step
   //   z inflow staging: element e = tid + q*NT of the [b][jj][ch][lane] block of step u
@@ -282,6 +302,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
           }
         }
     }
+    if (MASKED && vthread && ip1 >= 0 && ip1 < P.nx) cp_async<4>(&S->codes[rb][tid], cpsrc + (int64_t)t1 * 32);
     if (t1 < P.NU && !(P.dbg & 8)) {
 #pragma unroll
       for (int q = 0; q < (2 * NC * 32) / NT; ++q) {
@@ -373,6 +394,58 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     }
   };
 
+  // the same (band, chunk) on a patch that contains void cells or solid/void interface faces: every cell
+  // takes its upwind values through selects (interface inflow g instead of the neighbour) and void cells hold 0.
+  // cb[c] = code byte, g[c][axis] = interface inflow of cell c = A (0,0), B (1,0), C (0,1), D (1,1).
+  auto chunk_masked = [&](int b, int ch, const V2 (&r)[2][2], V2 (&m)[2][2][4], int rb, bool act, const uint32_t (&cb)[4],
+                          const T (&g)[4][3], const Ch *__restrict__ zrd, Ch *__restrict__ zwr) {
+    constexpr int NP = CP / 2;
+    const int h0 = (b * BTE2_P + ch * CP) / 2, cn = b * NCH + ch;
+    V2 yin[2][NP];
+#pragma unroll
+    for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+      for (int q = 0; q < NP; ++q) yin[kk][q] = mk2(shfl_up1<T>(c[1][kk][h0 + q].x), shfl_up1<T>(c[1][kk][h0 + q].y));
+    if (J == 0) {
+#pragma unroll
+      for (int kk = 0; kk < 2; ++kk) {
+        const Ch v = S->ybuf[rb][K][kk][cn];
+#pragma unroll
+        for (int q = 0; q < NP; ++q) yin[kk][q] = mk2(v.v[2 * q], v.v[2 * q + 1]);
+      }
+    }
+    const Ch z0 = zrd[cn * 32], z1 = zrd[(NC + cn) * 32];
+    if (!act) return;                                  // (shuffles above stay warp-convergent)
+    auto up = [&](uint32_t code, int axis, T gv, V2 v) { return (code >> (1 + fu[axis])) & 1u ? mk2(gv, gv) : v; };
+    auto keep = [&](uint32_t code, V2 v) { return (code & 1u) ? v : mk2((T)0, (T)0); };
+    Ch o0, o1;
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+      const int p = ch * CP + 2 * q;
+      const T(&kb)[8][BTE2_P] = CF.k[b0 + b];
+      const V2 inv = mk2(kb[0][p], kb[0][p + 1]), ax = mk2(kb[1][p], kb[1][p + 1]), ay = mk2(kb[2][p], kb[2][p + 1]),
+               az = mk2(kb[3][p], kb[3][p + 1]);
+      const V2 w0 = mk2(kb[4][p], kb[4][p + 1]), w1 = mk2(kb[5][p], kb[5][p + 1]), w2 = mk2(kb[6][p], kb[6][p + 1]),
+               w3 = mk2(kb[7][p], kb[7][p + 1]);
+      const V2 zq0 = mk2(z0.v[2 * q], z0.v[2 * q + 1]), zq1 = mk2(z1.v[2 * q], z1.v[2 * q + 1]);
+      V2 e00 = mul2(r[0][0], inv); e00 = fma2(ax, up(cb[0], 0, g[0][0], c[0][0][h0 + q]), e00);
+      e00 = fma2(ay, up(cb[0], 1, g[0][1], yin[0][q]), e00); e00 = fma2(az, up(cb[0], 2, g[0][2], zq0), e00); e00 = keep(cb[0], e00);
+      V2 e10 = mul2(r[1][0], inv); e10 = fma2(ax, up(cb[1], 0, g[1][0], c[1][0][h0 + q]), e10);
+      e10 = fma2(az, up(cb[1], 2, g[1][2], zq1), e10); e10 = fma2(ay, up(cb[1], 1, g[1][1], e00), e10); e10 = keep(cb[1], e10);
+      V2 e01 = mul2(r[0][1], inv); e01 = fma2(ax, up(cb[2], 0, g[2][0], c[0][1][h0 + q]), e01);
+      e01 = fma2(ay, up(cb[2], 1, g[2][1], yin[1][q]), e01); e01 = fma2(az, up(cb[2], 2, g[2][2], e00), e01); e01 = keep(cb[2], e01);
+      V2 e11 = mul2(r[1][1], inv); e11 = fma2(ax, up(cb[3], 0, g[3][0], c[1][1][h0 + q]), e11);
+      e11 = fma2(ay, up(cb[3], 1, g[3][1], e01), e11); e11 = fma2(az, up(cb[3], 2, g[3][2], e10), e11); e11 = keep(cb[3], e11);
+      c[0][0][h0 + q] = e00; c[1][0][h0 + q] = e10; c[0][1][h0 + q] = e01; c[1][1][h0 + q] = e11;
+      o0.v[2 * q] = e01.x; o0.v[2 * q + 1] = e01.y; o1.v[2 * q] = e11.x; o1.v[2 * q + 1] = e11.y;
+      acc2(m[0][0][0], w0, e00); acc2(m[0][0][1], w1, e00); acc2(m[0][0][2], w2, e00); acc2(m[0][0][3], w3, e00);
+      acc2(m[1][0][0], w0, e10); acc2(m[1][0][1], w1, e10); acc2(m[1][0][2], w2, e10); acc2(m[1][0][3], w3, e10);
+      acc2(m[0][1][0], w0, e01); acc2(m[0][1][1], w1, e01); acc2(m[0][1][2], w2, e01); acc2(m[0][1][3], w3, e01);
+      acc2(m[1][1][0], w0, e11); acc2(m[1][1][1], w1, e11); acc2(m[1][1][2], w2, e11); acc2(m[1][1][3], w3, e11);
+    }
+    zwr[cn * 32] = o0; zwr[(NC + cn) * 32] = o1;
+  };
+
   for (int t = 0; t < P.nsteps; ++t) {
     const int cur = t & 1, rb = t % R;
     const int ip = t - J - K;
@@ -398,7 +471,20 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
 #pragma unroll
       for (int jj = 0; jj < 2; ++jj) in[jj][kk] = S->inp[rb][kk][jj][tid];
 
-    const bool fast = __all_sync(FULL, act);
+    // masked grids: code bytes of the patch, oriented cell (jj,kk) -> byte (physical parities)
+    uint32_t cb[4] = {1u, 1u, 1u, 1u};
+    bool plain = true;
+    if (MASKED) {
+      const uint32_t code = act ? S->codes[rb][tid] : 0x01010101u;
+      plain = code == 0x01010101u;
+#pragma unroll
+      for (int cc = 0; cc < 4; ++cc) {
+        const int jj = cc & 1, kk = cc >> 1, pj = O.sy > 0 ? jj : 1 - jj, pk = O.sz > 0 ? kk : 1 - kk;
+        cb[cc] = (code >> (8 * (pj + 2 * pk))) & 0xffu;
+      }
+    }
+    const bool fast = __all_sync(FULL, act && plain);
+    const bool slowmask = MASKED && !__all_sync(FULL, plain);
     const Ch *__restrict__ zrd = K == 0 ? &S->zin0[rb][0][0][J] : &S->zex[cur][K - 1][0][0][J];
     Ch *__restrict__ zwr = &S->zex[cur ^ 1][K][0][0][J];
 #pragma unroll
@@ -411,7 +497,50 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
           const T rv = fma(bcx[b], in[jj][kk].x, bcy[b] * in[jj][kk].y);
           r[jj][kk] = mk2(rv, rv);
         }
-      if (fast) {
+      if (MASKED && slowmask) {
+        // physical cell indices of the patch, interface inflow per cell and axis (Eq. 5 / Eq. 6, lagged)
+        int64_t cph[4];
+        T g[4][3];
+#pragma unroll
+        for (int cc = 0; cc < 4; ++cc) {
+          const int jj = cc & 1, kk = cc >> 1;
+          const int i = O.sx > 0 ? ip : P.nx - 1 - ip, j = O.sy > 0 ? jp0 + jj : P.ny - 1 - jp0 - jj,
+                    k = O.sz > 0 ? kp0 + kk : P.nz - 1 - kp0 - kk;
+          cph[cc] = (int64_t)i + (int64_t)P.nx * (j + (int64_t)P.ny * k);
+#pragma unroll
+          for (int a = 0; a < 3; ++a) {
+            g[cc][a] = (T)0;
+            if (act && (cb[cc] & 1u) && ((cb[cc] >> (1 + fu[a])) & 1u))
+              g[cc][a] = P.iface_type == 0 ? (T)P.iface_e0[b0 + b]
+                                           : reinterpret_cast<const T *>(P.Gi)[(int64_t)P.iface[(int64_t)fu[a] * P.ncell + cph[cc]] * P.B + b0 + b];
+          }
+        }
+#pragma unroll
+        for (int ch = 0; ch < NCH; ++ch) chunk_masked(b, ch, r, m, rb, act, cb, g, zrd, zwr);
+        {
+          // outgoing hemispherical partial sums at solid/void faces (diffuse interface, Eq. 6)
+          if (act && P.iface_type == 1) {
+#pragma unroll
+            for (int cc = 0; cc < 4; ++cc) {
+              const int jj = cc & 1, kk = cc >> 1;
+              if (!(cb[cc] & 1u)) continue;
+#pragma unroll
+              for (int a = 0; a < 3; ++a) {
+                const int fd = fu[a] ^ 1;
+                if (!((cb[cc] >> (1 + fd)) & 1u)) continue;
+                double hsum = 0.0;
+#pragma unroll
+                for (int q = 0; q < BTE2_P / 2; ++q)
+                  hsum += P.wsa[2 * q][a] * (double)c[jj][kk][b * (BTE2_P / 2) + q].x + P.wsa[2 * q + 1][a] * (double)c[jj][kk][b * (BTE2_P / 2) + q].y;
+                const int bx = O.sx < 0, by = O.sy < 0, bz = O.sz < 0;
+                const int s2 = a == 0 ? (by | (bz << 1)) : (a == 1 ? (bx | (bz << 1)) : (bx | (by << 1)));
+                const int64_t fid = P.iface[(int64_t)fd * P.ncell + cph[cc]];
+                P.Hpart[(fid * P.B + b0 + b) * 4 + s2] = hsum;
+              }
+            }
+          }
+        }
+      } else if (fast) {
 #pragma unroll
         for (int ch = 0; ch < NCH; ++ch) chunk(std::true_type{}, b, ch, r, m, rb, cur, true, zrd, zwr);
       } else {
@@ -427,6 +556,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
         if (!(P.dbg & 2)) {
 #pragma unroll
           for (int jj = 0; jj < 2; ++jj) {
+            if (MASKED && !(cb[jj + 2 * kk] & 1u)) continue;      // void cell
             Bte2Mom<T> o;
             if (first) {
 #pragma unroll
@@ -490,7 +620,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
   if (tid == 0) st_release_gpu(P.prog + unit, ebase + 0xffff);
 }
 
-template <typename T, int W>
+template <typename T, int W, bool MASKED>
 __global__ void __launch_bounds__(W * 32) bte2_sweep_kernel(const __grid_constant__ Bte2Dev P,
                                                             const __grid_constant__ Bte2Coefs<T> CF) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -503,8 +633,8 @@ __global__ void __launch_bounds__(W * 32) bte2_sweep_kernel(const __grid_constan
     const int unit = s_unit;
     if (unit >= P.n_units) break;
     const Bte2Unit un = P.units[unit];
-    if (NBMAX == 2 && un.nb == 2) bte2_run_unit<T, NBMAX, W, D>(P, CF, un, smem_raw, unit);
-    else bte2_run_unit<T, 1, W, D>(P, CF, un, smem_raw, unit);
+    if (NBMAX == 2 && un.nb == 2) bte2_run_unit<T, NBMAX, W, D, MASKED>(P, CF, un, smem_raw, unit);
+    else bte2_run_unit<T, 1, W, D, MASKED>(P, CF, un, smem_raw, unit);
   }
 }
 
@@ -613,6 +743,17 @@ __global__ void bte2_ghost_kernel(const __grid_constant__ Bte2Dev P) {
       }
     }
   }
+  // interface faces: G = C dT_w / 4pi (isothermal) or (sum of the 4 outgoing octants' partial sums) / Pi_f (diffuse)
+  T *Gi = reinterpret_cast<T *>(P.Gi);
+  const int64_t ni = (int64_t)P.n_iface * P.B;
+  for (int64_t e = gtid; e < ni; e += gstride) {
+    const int64_t fid = e / P.B;
+    const int b = (int)(e % P.B);
+    if (P.iface_type == 0) { Gi[e] = (T)P.iface_e0[b]; continue; }
+    double H = 0.0;
+    for (int sl = 0; sl < 4; ++sl) H += P.Hpart[e * 4 + sl];
+    Gi[e] = (T)(H / P.Pi_face[P.iface_info[fid]]);
+  }
   if (gtid == 0) *P.ticket = 0;
 }
 
@@ -623,6 +764,7 @@ template <typename T>
 __global__ void __launch_bounds__(256, 4) bte2_update_kernel(const __grid_constant__ Bte2Dev P) {
   double sT = 0, mT = 0, sq = 0, mq = 0;
   for (int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; c < P.ncell; c += (int64_t)gridDim.x * blockDim.x) {
+    if (P.code && !(P.code[c] & 1)) continue;          // void cell: dT, q stay 0
     const int i = (int)(c % P.nx), j = (int)((c / P.nx) % P.ny), k = (int)(c / ((int64_t)P.nx * P.ny));
     int64_t sk[4];
 #pragma unroll
