@@ -338,7 +338,7 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
       U.b0 = g * NBmax; U.nb = std::min(NBmax, B - U.b0);
     }
     d.n_iface = nif; d.iface_type = p->interface_bc.type;
-    for (int b = 0; b < B; ++b) d.iface_e0[b] = pl.band[b] * p->interface_bc.dT_wall;
+    for (int b = 0; b < B; ++b) { d.iface_e0[b] = pl.band[b] * p->interface_bc.dT_wall; d.vband[b] = p->v[b]; }
     if (pl.masked2) {
       const size_t NPp = (size_t)(p->nz / 2) * d.nty * d.NU * 32;
       for (int cl = 0; cl < 4; ++cl) {

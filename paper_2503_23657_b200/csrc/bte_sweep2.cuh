@@ -93,6 +93,7 @@ struct Bte2Dev {
   double *Hpart;                    // [n_iface][B][4] outgoing hemispherical partial sums per octant slot
   int32_t n_iface, iface_type;
   double iface_e0[BTE2_MAXB];       // isothermal interface inflow C_b dT_w / 4pi
+  double vband[BTE2_MAXB];          // group velocities (to undo the v_b in the moment coefficients)
 };
 
 // ------------------------------------------------------------------ layouts (host + device)
@@ -473,10 +474,11 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
 
     // masked grids: code bytes of the patch, oriented cell (jj,kk) -> byte (physical parities)
     uint32_t cb[4] = {1u, 1u, 1u, 1u};
-    bool plain = true;
+    bool plain = true, live = act;                     // live: the patch holds at least one solid cell
     if (MASKED) {
       const uint32_t code = act ? S->codes[rb][tid] : 0x01010101u;
       plain = code == 0x01010101u;
+      live = act && (code & 0x01010101u) != 0;
 #pragma unroll
       for (int cc = 0; cc < 4; ++cc) {
         const int jj = cc & 1, kk = cc >> 1, pj = O.sy > 0 ? jj : 1 - jj, pk = O.sz > 0 ? kk : 1 - kk;
@@ -484,7 +486,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
       }
     }
     const bool fast = __all_sync(FULL, act && plain);
-    const bool slowmask = MASKED && !__all_sync(FULL, plain);
+    const bool slowmask = MASKED && __any_sync(FULL, live && !plain);
     const Ch *__restrict__ zrd = K == 0 ? &S->zin0[rb][0][0][J] : &S->zex[cur][K - 1][0][0][J];
     Ch *__restrict__ zwr = &S->zex[cur ^ 1][K][0][0][J];
 #pragma unroll
@@ -510,16 +512,20 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
 #pragma unroll
           for (int a = 0; a < 3; ++a) {
             g[cc][a] = (T)0;
-            if (act && (cb[cc] & 1u) && ((cb[cc] >> (1 + fu[a])) & 1u))
+            if (live && (cb[cc] & 1u) && ((cb[cc] >> (1 + fu[a])) & 1u))
               g[cc][a] = P.iface_type == 0 ? (T)P.iface_e0[b0 + b]
-                                           : reinterpret_cast<const T *>(P.Gi)[(int64_t)P.iface[(int64_t)fu[a] * P.ncell + cph[cc]] * P.B + b0 + b];
+                                           : reinterpret_cast<const T *>(P.Gi)[(int64_t)__ldg(P.iface + (int64_t)fu[a] * P.ncell + cph[cc]) * P.B + b0 + b];
           }
         }
 #pragma unroll
-        for (int ch = 0; ch < NCH; ++ch) chunk_masked(b, ch, r, m, rb, act, cb, g, zrd, zwr);
+        for (int ch = 0; ch < NCH; ++ch) chunk_masked(b, ch, r, m, rb, live, cb, g, zrd, zwr);
         {
           // outgoing hemispherical partial sums at solid/void faces (diffuse interface, Eq. 6)
-          if (act && P.iface_type == 1) {
+          uint32_t anydn = 0;
+#pragma unroll
+          for (int cc = 0; cc < 4; ++cc)
+            if (cb[cc] & 1u) anydn |= cb[cc] & ((2u << (fu[0] ^ 1)) | (2u << (fu[1] ^ 1)) | (2u << (fu[2] ^ 1)));
+          if (P.iface_type == 1 && live && anydn != 0) {
 #pragma unroll
             for (int cc = 0; cc < 4; ++cc) {
               const int jj = cc & 1, kk = cc >> 1;
@@ -528,10 +534,13 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
               for (int a = 0; a < 3; ++a) {
                 const int fd = fu[a] ^ 1;
                 if (!((cb[cc] >> (1 + fd)) & 1u)) continue;
-                double hsum = 0.0;
+                // sum_p w_p |s_p,a| e_p in the compute type with the moment coefficients v_b w |s_a| (<= 16 terms of
+                // one sign pattern), divided by v_b; the sum over the 4 outgoing octants is fp64 (ghost kernel)
+                V2 hs = mk2((T)0, (T)0);
 #pragma unroll
                 for (int q = 0; q < BTE2_P / 2; ++q)
-                  hsum += P.wsa[2 * q][a] * (double)c[jj][kk][b * (BTE2_P / 2) + q].x + P.wsa[2 * q + 1][a] * (double)c[jj][kk][b * (BTE2_P / 2) + q].y;
+                  hs = fma2(mk2(CF.k[b0 + b][5 + a][2 * q], CF.k[b0 + b][5 + a][2 * q + 1]), c[jj][kk][b * (BTE2_P / 2) + q], hs);
+                const double hsum = ((double)hs.x + (double)hs.y) / P.vband[b0 + b];
                 const int bx = O.sx < 0, by = O.sy < 0, bz = O.sz < 0;
                 const int s2 = a == 0 ? (by | (bz << 1)) : (a == 1 ? (bx | (bz << 1)) : (bx | (by << 1)));
                 const int64_t fid = P.iface[(int64_t)fd * P.ncell + cph[cc]];
@@ -545,7 +554,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
         for (int ch = 0; ch < NCH; ++ch) chunk(std::true_type{}, b, ch, r, m, rb, cur, true, zrd, zwr);
       } else {
 #pragma unroll
-        for (int ch = 0; ch < NCH; ++ch) chunk(std::false_type{}, b, ch, r, m, rb, cur, act, zrd, zwr);
+        for (int ch = 0; ch < NCH; ++ch) chunk(std::false_type{}, b, ch, r, m, rb, cur, live, zrd, zwr);
       }
     }
 

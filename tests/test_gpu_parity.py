@@ -112,6 +112,29 @@ def test_fast_path_tile_heights(bte, warps, monkeypatch):
     check(bte, p, 4, precision=W.FP64)
 
 
+@pytest.mark.parametrize("seed", range(6))
+def test_masked_grids_on_the_fast_path(bte, seed):
+    """Voxel masks on the fast sweep kernel (even ny, nz, 16 directions per octant): random masks with isothermal or
+    diffuse interfaces, periodic axes whose wrap may land on void cells, both precisions."""
+    p = W.random_problem(seed, dim=3, shape=(14 + seed, 10 + 2 * seed, 8 + 2 * (seed % 3)), masked=True,
+                         periodic_axis=(seed % 3 if seed % 2 else None),
+                         interface_type=(W.BC_DIFFUSE if seed % 2 == 0 else W.BC_ISOTHERMAL), n_polar=8, n_azimuth=16)
+    assert bte.Solver(p).kernel_path == 2
+    check(bte, p, 12, precision=W.FP64, checkpoints=(1, 3))
+    check(bte, p, 12, precision=W.FP32_STORE_FP64_ACC)
+
+
+def test_finfet_mask_fast_vs_generic(bte, monkeypatch):
+    """Config 3 (fin + slab, diffuse interfaces, periodic x) at a size with several z tiles on both kernel paths."""
+    p = W.config(3, grid=(36, 68, 40))
+    assert bte.Solver(p).kernel_path == 2
+    check(bte, p, 20, checkpoints=(1, 5))
+    check(bte, p, 6, precision=W.FP64, checkpoints=(1,))
+    monkeypatch.setenv("BTE_FORCE_GENERIC", "1")
+    assert bte.Solver(p).kernel_path == 1
+    check(bte, p, 6, precision=W.FP64, checkpoints=(1,))
+
+
 # ---------------------------------------------------------------- random problems: every BC mix
 @pytest.mark.parametrize("seed", range(8))
 @pytest.mark.parametrize("dim", [1, 2, 3])
