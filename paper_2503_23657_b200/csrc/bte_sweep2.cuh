@@ -1,5 +1,5 @@
-// Fast path ("v2") of the B200 phonon-BTE sweep: 3-D, unmasked or masked-by-fallback, 16 directions per
-// octant, mirror-symmetric quadrature, <= 16 bands.  DESIGN.md "Kernels / sweep v2".
+// Fast path of the B200 phonon-BTE sweep: 3-D, even ny / nz, all-solid or voxel-masked, 16 directions per
+// octant, mirror-symmetric quadrature, <= 16 bands.  DESIGN.md section 6.
 //
 // Mapping.  One CTA = W warps sweeps one tile = 64 (y') x 2W (z') rows along x' for one octant and
 // one band group (NB = 1 or 2 bands x 16 directions).  Thread (J = lane, K = warp) owns the 2x2
