@@ -295,8 +295,8 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
   pl.v2 = v2;
   if (v2) {
     Bte2Dev &d = pl.d2;
-    int W = (p->nz >= 48 && dv.fp32) ? 8 : 4;   // fp64 staging buffers of 8 warps do not fit shared memory
-    if (const char *e = std::getenv("BTE_V2_W")) { const int w = std::atoi(e); if (w == 4 || (w == 8 && dv.fp32)) W = w; }
+    int W = p->nz >= 48 ? 8 : 4;
+    if (const char *e = std::getenv("BTE_V2_W")) { const int w = std::atoi(e); if (w == 4 || w == 8) W = w; }
     d.nx = p->nx; d.ny = p->ny; d.nz = p->nz; d.B = B; d.W = W;
     d.nty = (p->ny + 63) / 64; d.ntz = (p->nz + 2 * W - 1) / (2 * W); d.NU = p->nx + 31;
     d.nsteps = p->nx + 31 + W - 1;
@@ -467,7 +467,7 @@ void order_units2(Plan &pl, int slots) {
     const int lag[3] = {33, W + 1, 1};
     double a = 0;
     for (int k = 0; k < 3; ++k)
-      if (deps[k] >= 0) a = std::max(a, start[deps[k]] + (lag[k] + BTE2_DIST(W) + pl.d2.slack + pl.d2.pub_mask + 1) * steptime[deps[k]]);
+      if (deps[k] >= 0) a = std::max(a, start[deps[k]] + (lag[k] + (pl.dev.fp32 ? BTE2_DIST(W, float) : BTE2_DIST(W, double)) + pl.d2.slack + pl.d2.pub_mask + 1) * steptime[deps[k]]);
     return a;
   };
   typedef std::pair<double, int> Key;
@@ -594,7 +594,7 @@ bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t
 template <typename T, int W>
 bte_status setup_sweep2_W(bte_solver *h) {
   Plan &pl = h->pl;
-  pl.smem2 = sizeof(Bte2Smem<T, sizeof(T) == 4 ? 2 : 1, W, BTE2_DIST(W)>);
+  pl.smem2 = sizeof(Bte2Smem<T, sizeof(T) == 4 ? 2 : 1, W, BTE2_DIST(W, T)>);
   int occ = 0;
   if (pl.masked2) {
     CK(cudaFuncSetAttribute(bte2_sweep_kernel<T, W, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem2));

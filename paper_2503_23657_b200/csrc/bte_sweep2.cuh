@@ -29,7 +29,8 @@
 #define BTE2_P 16         // directions per octant
 #define BTE2_MAXB 16      // bands in the parameter table
 #define BTE2_PUB 8        // progress is published every PUB steps
-#define BTE2_DIST(W) ((W) >= 8 ? 2 : 1)   // cp.async prefetch distance in steps (1 lets two 4-warp CTAs share an SM)
+#define BTE2_DIST(W, T) (((W) >= 8 && sizeof(T) == 4) ? 2 : 1)   // cp.async prefetch distance in steps (shared-memory budget)
+#define BTE2_MDIST(T) (sizeof(T) == 4 ? 1 : 0)   // same for the moment accumulator (fp64: fetched in the step that adds to it)
 #define BTE2_SLACK 0      // extra steps a unit lets the units it follows get ahead before it starts
 #define BTE2_TYROWS 64    // tile rows along y' (32 lanes x 2)
 
@@ -185,7 +186,7 @@ template <typename T, int NB, int W, int D> struct Bte2Smem {
   Ch zin0[D + 1][2][NC][32];         // staged z inflow plane of warp 0
   Ch ybuf[D + 1][W][2][NC];          // [ring][warp][kk][chunk]: y inflow of lane 0
   Ch yst[2][W][2 * NC];              // [parity][warp][kk*NC + chunk]: jj=1 rows of lane Jl, copied out one step later
-  Bte2Mom<T> mold[2][2][2][W * 32];  // [parity][kk][jj][tid] previous content of the moment accumulator
+  Bte2Mom<T> mold[BTE2_MDIST(T) + 1][2][2][W * 32];  // [ring][kk][jj][tid] previous content of the moment accumulator
   Bte2Pair<T> inp[D + 1][2][2][W * 32];    // [ring][kk][jj][tid] (dT, Q/sumC) of the cell
   uint32_t codes[D + 1][W * 32];           // [ring][tid] cell bytes of the thread's patch (masked grids only)
 };
@@ -269,7 +270,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
           const int64_t ci = cbase[kk] + jj * 32 + (int64_t)t1 * 64;
 #pragma unroll
           for (int h = 0; h < (int)sizeof(Bte2Mom<T>) / 16; ++h)
-            cp_async<16>(reinterpret_cast<char *>(&S->mold[t1 & 1][kk][jj][tid]) + 16 * h, reinterpret_cast<const char *>(M + ci) + 16 * h);
+            cp_async<16>(reinterpret_cast<char *>(&S->mold[t1 % (BTE2_MDIST(T) + 1)][kk][jj][tid]) + 16 * h, reinterpret_cast<const char *>(M + ci) + 16 * h);
         }
     }
   };
@@ -337,7 +338,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
   __syncthreads();
 #pragma unroll
   for (int t1 = 0; t1 < D; ++t1) {
-    if (t1 == 0) prefetch_m(0);
+    if (t1 == 0 && BTE2_MDIST(T) == 1) prefetch_m(0);
     prefetch(t1); cp_async_commit();
   }
   cp_async_wait<D - 1>();
@@ -451,7 +452,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     const int cur = t & 1, rb = t % R;
     const int ip = t - J - K;
     const bool act = vthread && ip >= 0 && ip < P.nx;
-    prefetch_m(t + 1);
+    prefetch_m(t + BTE2_MDIST(T));
     cp_async_commit();
     prefetch(t + D);
     cp_async_commit();
@@ -571,7 +572,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
 #pragma unroll
               for (int q = 0; q < 4; ++q) o.v[q] = m[jj][kk][q].x + m[jj][kk][q].y;
             } else {
-              const Bte2Mom<T> old = S->mold[cur][kk][jj][tid];
+              const Bte2Mom<T> old = S->mold[t % (BTE2_MDIST(T) + 1)][kk][jj][tid];
 #pragma unroll
               for (int q = 0; q < 4; ++q) o.v[q] = old.v[q] + (m[jj][kk][q].x + m[jj][kk][q].y);
             }
@@ -633,7 +634,7 @@ template <typename T, int W, bool MASKED>
 __global__ void __launch_bounds__(W * 32) bte2_sweep_kernel(const __grid_constant__ Bte2Dev P,
                                                             const __grid_constant__ Bte2Coefs<T> CF) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  constexpr int NBMAX = sizeof(T) == 4 ? 2 : 1, D = BTE2_DIST(W);
+  constexpr int NBMAX = sizeof(T) == 4 ? 2 : 1, D = BTE2_DIST(W, T);
   __shared__ int s_unit;
   for (;;) {
     __syncthreads();
