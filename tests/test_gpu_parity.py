@@ -283,3 +283,21 @@ def test_config4_replica_converged_state(bte, prec):
     p = W.config(4, grid=(32, 16, 16))
     out = check(bte, p, 400, precision=prec, checkpoints=(100,))
     assert out[-1][3][0] < 1e-5          # oracle eps_T: well converged
+
+
+@pytest.mark.slow
+def test_progress_epoch_wraps_without_hanging(bte):
+    """The per-unit progress words carry the iteration number in their upper bits and are re-zeroed every 30000
+    iterations; run a tiny fast-path problem across that boundary (it is long converged by then)."""
+    p = W.config(2, grid=(8, 8, 8))
+    g = bte.Solver(p)
+    assert g.kernel_path == 2
+    g.iterate(29990)
+    a = g.temperature().clone()
+    g.iterate(25)                      # crosses iteration 30000
+    b = g.temperature()
+    assert g.iterations_done == 30015
+    assert bool(((a - b).abs() <= 1e-9 * a.abs().max()).all())
+    import oracle
+    ref = oracle.RefSolver(p); ref.iterate(3000)          # converged reference (fixed point)
+    assert np.abs(b.cpu().numpy() - ref.temperature()).max() <= 1e-8 * np.abs(ref.temperature()).max()
