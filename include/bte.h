@@ -125,6 +125,12 @@ int32_t bte_kernel_path(const bte_solver *h);
  * [3]=wavefront steps summed over units, [4]=thread-slot updates issued per sweep (occupancy
  * denominator: useful updates / this), [5]=bytes of workspace in use */
 void bte_schedule_info(const bte_solver *h, int64_t out[6]);
+/* Host-only view of the plan bte_create would build (no CUDA call): out[0] = kernel path (1 / 2), [1] = work
+ * units per sweep, [2] = 1 if the ticket order is topological (every unit comes after the units it follows, and
+ * each dependency points at the right neighbour tile / band group) when simulated for `resident_ctas` CTAs,
+ * [3] = wavefront steps per unit, [4] = warps per CTA, [5] = band groups, [6] = 1 if voxel-masked, [7] = workspace
+ * bytes.  Returns the status bte_create would return for an invalid problem. */
+bte_status bte_plan_info(const bte_problem *p, int32_t resident_ctas, int64_t out[8]);
 void bte_destroy(bte_solver *h);
 const char *bte_status_string(bte_status s);
 int32_t bte_last_cuda_error(void);

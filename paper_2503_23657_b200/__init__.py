@@ -32,7 +32,7 @@ BTE_FP64, BTE_FP32_STORE_FP64_ACC = 0, 1
 EXPORTS = ["bte_workspace_bytes", "bte_create", "bte_iterate", "bte_get_temperature", "bte_get_heat_flux",
            "bte_set_temperature", "bte_residual", "bte_solve_host", "bte_set_sweep_timing",
            "bte_get_sweep_timing", "bte_updates_per_sweep",
-           "bte_iterations_done", "bte_kernel_launches_per_iteration", "bte_kernel_path", "bte_schedule_info", "bte_destroy",
+           "bte_iterations_done", "bte_kernel_launches_per_iteration", "bte_kernel_path", "bte_plan_info", "bte_schedule_info", "bte_destroy",
            "bte_status_string", "bte_last_cuda_error"]
 
 
@@ -99,6 +99,7 @@ def lib():
         L.bte_iterations_done.restype = i64
         L.bte_kernel_launches_per_iteration.argtypes = [vp]
         L.bte_kernel_launches_per_iteration.restype = i32
+        L.bte_plan_info.argtypes = [C.POINTER(_Problem), i32, C.POINTER(i64)]
         L.bte_kernel_path.argtypes = [vp]
         L.bte_kernel_path.restype = i32
         L.bte_schedule_info.argtypes = [vp, C.POINTER(i64)]
@@ -137,6 +138,18 @@ def _marshal(p, precision=None):
 def bte_workspace_bytes(p, precision=None) -> int:
     pr, _keep = _marshal(p, precision)
     return int(lib().bte_workspace_bytes(C.byref(pr)))
+
+
+def bte_plan_info(p, resident_ctas=148, precision=None):
+    """Host-only plan summary (no GPU needed)."""
+    pr, _keep = _marshal(p, precision)
+    out = (C.c_int64 * 8)()
+    rc = lib().bte_plan_info(C.byref(pr), int(resident_ctas), out)
+    if rc:
+        raise BteError(rc, "bte_plan_info")
+    keys = ["kernel_path", "work_units", "order_ok", "steps_per_unit", "warps_per_cta", "band_groups", "masked",
+            "workspace_bytes"]
+    return dict(zip(keys, [int(x) for x in out]))
 
 
 class Solver:

@@ -824,6 +824,37 @@ bte_status bte_solve_host(bte_solver *h, const double *Q_host, int32_t n, int32_
   return BTE_OK;
 }
 
+bte_status bte_plan_info(const bte_problem *p, int32_t resident_ctas, int64_t out[8]) {
+  if (!out) return BTE_ERR_INVALID_ARG;
+  Plan pl;
+  bte_status st = build_plan(p, pl);
+  if (st != BTE_OK) return st;
+  for (int i = 0; i < 8; ++i) out[i] = 0;
+  out[0] = pl.v2 ? 2 : 1;
+  out[7] = (int64_t)bind(pl, nullptr);
+  if (!pl.v2) {
+    out[1] = pl.dev.n_units; out[3] = pl.dev.nx + 31 + pl.dev.TZ - 1; out[4] = pl.dev.TZ;
+    bool topo = true;
+    for (size_t u = 0; u < pl.units.size(); ++u)
+      for (int d : {pl.units[u].dep_y, pl.units[u].dep_z, pl.units[u].dep_prev}) topo = topo && d < (int)u;
+    out[2] = topo;
+    return BTE_OK;
+  }
+  order_units2(pl, std::max(resident_ctas, 1));
+  bool topo = true, same = true;
+  for (size_t u = 0; u < pl.units2.size(); ++u) {
+    const Bte2Unit &U = pl.units2[u];
+    for (int d : {U.dep_y, U.dep_z, U.dep_prev}) topo = topo && d < (int)u;
+    if (U.dep_y >= 0) { const Bte2Unit &D = pl.units2[U.dep_y]; same = same && D.oct == U.oct && D.g == U.g && D.ty == U.ty - 1 && D.tz == U.tz; }
+    if (U.dep_z >= 0) { const Bte2Unit &D = pl.units2[U.dep_z]; same = same && D.oct == U.oct && D.g == U.g && D.ty == U.ty && D.tz == U.tz - 1; }
+    if (U.dep_prev >= 0) { const Bte2Unit &D = pl.units2[U.dep_prev]; same = same && D.oct == U.oct && D.g == U.g - 1 && D.ty == U.ty && D.tz == U.tz; }
+  }
+  out[1] = pl.d2.n_units; out[2] = topo && same; out[3] = pl.d2.nsteps; out[4] = pl.d2.W;
+  out[5] = (pl.d2.B + (pl.dev.fp32 ? 2 : 1) - 1) / (pl.dev.fp32 ? 2 : 1);
+  out[6] = pl.masked2;
+  return BTE_OK;
+}
+
 int64_t bte_updates_per_sweep(const bte_solver *h) {
   if (!h) return 0;
   return h->pl.dev.nsolid * h->pl.dev.B * (int64_t)h->pl.dev.n_dirs;
