@@ -205,7 +205,6 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
   dv.max_items = max_items;
   dv.nHslot = 4 * max_chunk;
   pl.item_coef.assign((size_t)8 * max_items, 0);
-  std::map<std::string, int32_t> seen;
   for (int o = 0; o < 8; ++o) {
     const BteOct &O = dv.oct[o];
     for (int b = 0; b < B; ++b) for (int c = 0; c < O.nchunk; ++c) {
@@ -224,14 +223,18 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
         r[4] = p->w[d];
         for (int a = 0; a < 3; ++a) r[5 + a] = p->w[d] * std::fabs(p->s[3 * d + a]);
       }
-      const std::string k((const char *)blk, sizeof blk);
-      auto it = seen.find(k);
-      int32_t off;
-      if (it == seen.end()) {
+      // reuse an existing block that agrees to rounding (mirrored direction cosines differ in the last bits)
+      int32_t off = -1;
+      for (size_t e = 0; e + BTE_P * BTE_NCOEF <= pl.coef.size() && off < 0; e += BTE_P * BTE_NCOEF) {
+        bool eq = true;
+        for (int c = 0; c < BTE_P * BTE_NCOEF && eq; ++c)
+          eq = std::fabs(pl.coef[e + c] - blk[c]) <= 1e-13 * std::max(std::fabs(blk[c]), 1e-300);
+        if (eq) off = (int32_t)e;
+      }
+      if (off < 0) {
         off = (int32_t)pl.coef.size();
         pl.coef.insert(pl.coef.end(), blk, blk + BTE_P * BTE_NCOEF);
-        seen.emplace(k, off);
-      } else off = it->second;
+      }
       pl.item_coef[(size_t)o * max_items + b * O.nchunk + c] = off;
     }
   }
