@@ -559,6 +559,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
       }
     }
 
+    if (BTE2_MDIST(T) == 0) cp_async_wait<D - 1>();   // the accumulator content fetched in THIS step has landed
     if (act) {
       // (b) moments of this band group into the octant accumulator (one owner per cell and group)
 #pragma unroll
