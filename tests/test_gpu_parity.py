@@ -301,3 +301,22 @@ def test_progress_epoch_wraps_without_hanging(bte):
     import oracle
     ref = oracle.RefSolver(p); ref.iterate(3000)          # converged reference (fixed point)
     assert np.abs(b.cpu().numpy() - ref.temperature()).max() <= 1e-8 * np.abs(ref.temperature()).max()
+
+
+@pytest.mark.parametrize("warps", ["4", "8"])
+@pytest.mark.parametrize("prec", [W.FP64, W.FP32_STORE_FP64_ACC])
+@pytest.mark.parametrize("k", [3, 4])
+def test_repeated_runs_are_bitwise_identical(bte, k, prec, warps, monkeypatch):
+    """Race detector for the tile pipeline (inter-tile progress flags, staged faces, accumulator hand-over between band
+    groups): several y and z tiles, every run of the same problem must give the same bits."""
+    monkeypatch.setenv("BTE_V2_W", warps)
+    p = W.config(k, grid=(45, 130, 36) if k == 4 else (40, 68, 40))
+    ref = None
+    for _ in range(5):
+        g = bte.Solver(p, precision=prec)
+        assert g.kernel_path == 2
+        g.iterate(4)
+        t = g.temperature()
+        if ref is None:
+            ref = t.clone()
+        assert bool((t == ref).all())
