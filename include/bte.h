@@ -116,9 +116,10 @@ bte_status bte_get_sweep_timing(bte_solver *h, double *total_ms, int64_t *launch
 int64_t bte_updates_per_sweep(const bte_solver *h); /* solid cells * n_bands * n_dirs */
 int64_t bte_iterations_done(const bte_solver *h);
 int32_t bte_kernel_launches_per_iteration(const bte_solver *h);
-/* Which sweep kernel serves this problem: 2 = fast path (3-D, even ny and nz, all-solid or voxel-masked, 16
- * directions in each octant with mirror-symmetric |s|, w tables, <= 16 bands), 1 = generic path (everything else:
- * 1-D / 2-D, odd ny / nz, other quadratures).  Both compute the same iteration; the environment variable
+/* Which sweep kernel serves this problem: 2 = fast path (3-D with even ny and nz, or 2-D with even ny -- run as a
+ * slab of two identical layers without z coupling; all-solid or voxel-masked; 16 directions in each octant with
+ * mirror-symmetric |s|, w tables; <= 16 bands), 1 = generic path (everything else: 1-D, odd ny / nz, other
+ * quadratures).  Both compute the same iteration; the environment variable
  * BTE_FORCE_GENERIC=1 (read by bte_create) forces 1 for testing. */
 int32_t bte_kernel_path(const bte_solver *h);
 /* schedule facts for reporting: out[0]=work units per sweep, [1]=CTAs launched, [2]=threads per CTA,

@@ -46,6 +46,8 @@ struct Plan {
   size_t gf_elems = 0;
   // fast path (bte_sweep2.cuh)
   bool v2 = false, masked2 = false;
+  int layers = 1;                        // 2: a 2-D problem run as a two-layer 3-D slab on the fast path
+  int64_t user_ncell = 0, user_nsolid = 0;
   std::vector<uint32_t> codeP[4];
   Bte2Dev d2{};
   std::vector<Bte2Unit> units2;
@@ -58,7 +60,7 @@ struct Plan {
 
 size_t align_up(size_t x) { return (x + 255) & ~size_t(255); }
 
-bte_status build_plan(const bte_problem *p, Plan &pl) {
+bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
   if (!p) return BTE_ERR_INVALID_ARG;
   if (p->nx < 1 || p->ny < 1 || p->nz < 1 || p->dim < 1 || p->dim > 3) return BTE_ERR_INVALID_ARG;
   if ((p->dim < 3 && p->nz != 1) || (p->dim < 2 && p->ny != 1)) return BTE_ERR_INVALID_ARG;
@@ -308,7 +310,7 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
     if (const char *e = std::getenv("BTE_V2_PUB")) { const int v = std::atoi(e); if (v == 4 || v == 8 || v == 16 || v == 32) d.pub_mask = v - 1; }
     if (const char *e = std::getenv("BTE_V2_SLACK")) { const int v = std::atoi(e); if (v >= 0 && v <= 256) d.slack = v; }
     d.NS = (int64_t)p->nz * d.nty * d.NU * 64;
-    d.ncell = N; d.inv_sumCtau = dv.inv_sumCtau;
+    d.ncell = N; d.src_mod = N; d.inv_sumCtau = dv.inv_sumCtau;
     const int NBmax = dv.fp32 ? 2 : 1, G = (B + NBmax - 1) / NBmax;
     for (int b = 0; b < B; ++b) {
       const double *blk = pl.coef.data() + pl.item_coef[b];
@@ -369,6 +371,32 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
       d.gf_off[f] = off; off += na * nb * B;
     }
     pl.steps_total = (int64_t)pl.units2.size() * d.nsteps;
+  }
+  return BTE_OK;
+}
+
+// 2-D problems (dim 2, nz 1) have no z coupling; on the fast path they run as a 3-D slab of two identical layers
+// with a z spacing so large that the z coefficient vanishes (c_z = v tau |s_z| / dz -> 0), isothermal z faces
+// whose inflow is then multiplied by 0.  Layer 0 is what the caller sees; the second layer is redundant work
+// (not counted in bte_updates_per_sweep) that buys the tiled, register-resident sweep instead of the generic one.
+bte_status build_plan(const bte_problem *p, Plan &pl) {
+  bte_status st = build_plan_impl(p, pl);
+  pl.user_ncell = pl.dev.ncell; pl.user_nsolid = pl.dev.nsolid;
+  if (st != BTE_OK || pl.v2 || p->dim != 2 || p->ny % 2 != 0) return st;
+  if (const char *e = std::getenv("BTE_FORCE_GENERIC")) if (e[0] == '1') return st;
+  const size_t N = (size_t)p->nx * p->ny;
+  std::vector<uint8_t> mask2;
+  std::vector<double> Q2;
+  bte_problem q = *p;
+  q.dim = 3; q.nz = 2; q.dz = 1e300;
+  q.face_bc[4].type = q.face_bc[5].type = BTE_BC_ISOTHERMAL;
+  q.face_bc[4].dT_wall = q.face_bc[5].dT_wall = 0.0;
+  if (p->solid_mask) { mask2.assign(p->solid_mask, p->solid_mask + N); mask2.insert(mask2.end(), p->solid_mask, p->solid_mask + N); q.solid_mask = mask2.data(); }
+  if (p->Q) { Q2.assign(p->Q, p->Q + N); Q2.insert(Q2.end(), p->Q, p->Q + N); q.Q = Q2.data(); }
+  Plan p3;
+  if (build_plan_impl(&q, p3) == BTE_OK && p3.v2) {
+    p3.layers = 2; p3.user_ncell = pl.dev.ncell; p3.user_nsolid = pl.dev.nsolid;
+    pl = std::move(p3);
   }
   return BTE_OK;
 }
@@ -669,6 +697,7 @@ bte_status bte_create(const bte_problem *p, void *d_workspace, size_t bytes, voi
   if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255) || bytes < need) { delete h; return BTE_ERR_WORKSPACE; }
   h->ws = static_cast<unsigned char *>(d_workspace);
   bind(h->pl, h->ws);
+  h->pl.d2.src_mod = h->pl.user_ncell;
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   Plan &pl = h->pl;
   BteDev &dv = pl.dev;
@@ -736,15 +765,16 @@ bte_status bte_iterate(bte_solver *h, int32_t n, void *cuda_stream) {
 
 bte_status bte_get_temperature(bte_solver *h, double *d_out, void *cuda_stream) {
   if (!h || !d_out) return BTE_ERR_INVALID_ARG;
-  CK(cudaMemcpyAsync(d_out, h->pl.dev.dT, (size_t)h->pl.dev.ncell * 8, cudaMemcpyDeviceToDevice,
+  CK(cudaMemcpyAsync(d_out, h->pl.dev.dT, (size_t)h->pl.user_ncell * 8, cudaMemcpyDeviceToDevice,
                      static_cast<cudaStream_t>(cuda_stream)));
   return BTE_OK;
 }
 
 bte_status bte_get_heat_flux(bte_solver *h, double *d_out, void *cuda_stream) {
   if (!h || !d_out) return BTE_ERR_INVALID_ARG;
-  CK(cudaMemcpyAsync(d_out, h->pl.dev.q, (size_t)h->pl.dev.ncell * 24, cudaMemcpyDeviceToDevice,
-                     static_cast<cudaStream_t>(cuda_stream)));
+  for (int c = 0; c < 3; ++c)
+    CK(cudaMemcpyAsync(d_out + c * h->pl.user_ncell, h->pl.dev.q + c * h->pl.dev.ncell, (size_t)h->pl.user_ncell * 8,
+                       cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(cuda_stream)));
   return BTE_OK;
 }
 
@@ -807,7 +837,7 @@ bte_status bte_solve_host(bte_solver *h, const double *Q_host, int32_t n, int32_
   Plan &pl = h->pl;
   BteDev &dv = pl.dev;
   if (Q_host) {
-    CK(cudaMemcpyAsync(dv.Qphys, Q_host, (size_t)dv.ncell * 8, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(dv.Qphys, Q_host, (size_t)pl.user_ncell * 8, cudaMemcpyHostToDevice, s));
     bte_status st = skew(h, dv.Qphys, 1.0 / pl.sumC, 0, s);
     if (st != BTE_OK) return st;
   }
@@ -821,8 +851,10 @@ bte_status bte_solve_host(bte_solver *h, const double *Q_host, int32_t n, int32_
   }
   bte_status st = bte_iterate(h, n, cuda_stream);
   if (st != BTE_OK) return st;
-  CK(cudaMemcpyAsync(dT_host, dv.dT, (size_t)dv.ncell * 8, cudaMemcpyDeviceToHost, s));
-  if (q_host) CK(cudaMemcpyAsync(q_host, dv.q, (size_t)dv.ncell * 24, cudaMemcpyDeviceToHost, s));
+  CK(cudaMemcpyAsync(dT_host, dv.dT, (size_t)pl.user_ncell * 8, cudaMemcpyDeviceToHost, s));
+  if (q_host)
+    for (int c = 0; c < 3; ++c)
+      CK(cudaMemcpyAsync(q_host + c * pl.user_ncell, dv.q + c * dv.ncell, (size_t)pl.user_ncell * 8, cudaMemcpyDeviceToHost, s));
   CK(cudaStreamSynchronize(s));
   return BTE_OK;
 }
@@ -860,7 +892,7 @@ bte_status bte_plan_info(const bte_problem *p, int32_t resident_ctas, int64_t ou
 
 int64_t bte_updates_per_sweep(const bte_solver *h) {
   if (!h) return 0;
-  return h->pl.dev.nsolid * h->pl.dev.B * (int64_t)h->pl.dev.n_dirs;
+  return h->pl.user_nsolid * h->pl.dev.B * (int64_t)h->pl.dev.n_dirs;
 }
 int64_t bte_iterations_done(const bte_solver *h) { return h ? h->iters : 0; }
 int32_t bte_kernel_launches_per_iteration(const bte_solver *h) { return h ? h->launches_per_iter : 0; }

@@ -81,7 +81,7 @@ struct Bte2Dev {
   double *dT, *q, *qmag, *red;      // fp64 outputs in physical layout; residual partials
   int32_t n_red_blocks, pub_mask;   // progress is published when (t & pub_mask) == pub_mask
   int32_t slack, fill_iso;          // fill_iso: (re)write the constant isothermal ghost planes (first iteration only)
-  int64_t ncell;
+  int64_t ncell, src_mod;            // src_mod: cells of the caller's field (2-D problems run as two layers)
   double inv_sumCtau;
   // voxel masks (all null / 0 when every cell is solid).  Cell byte: bit0 solid, bit 1+f: the neighbour across
   // face f (x-,x+,y-,y+,z-,z+) is a solid/void interface (or a periodic wrap onto a void cell).
@@ -823,9 +823,9 @@ __global__ void bte2_skew_kernel(const __grid_constant__ Bte2Dev P, const double
     for (int cl = 0; cl < 4; ++cl) {
       Bte2Pair<T> *d = reinterpret_cast<Bte2Pair<T> *>(P.dTQ[cl]) +
                        sk2_index(P.nty, P.NU, (cl & 1) ? P.nx - 1 - i : i, (cl & 2) ? P.ny - 1 - j : j, k);
-      if (which == 0) d->y = (T)(src[c] * scale); else d->x = (T)src[c];
+      if (which == 0) d->y = (T)(src[c % P.src_mod] * scale); else d->x = (T)src[c % P.src_mod];
     }
-    if (which == 1) P.dT[c] = src[c];
+    if (which == 1) P.dT[c] = src[c % P.src_mod];
   }
 }
 #endif  // __CUDACC__

@@ -13,7 +13,7 @@ def _built():
     bte.build()
 
 
-@pytest.mark.parametrize("k,grid,path", [(0, None, 1), (1, None, 1), (2, (64, 64, 64), 2), (3, (128, 64, 64), 2),
+@pytest.mark.parametrize("k,grid,path", [(0, None, 1), (1, None, 2), (1, (45, 71, 1), 1), (2, (64, 64, 64), 2), (3, (128, 64, 64), 2),
                                          (4, (256, 128, 128), 2), (2, (19, 37, 21), 1), (4, (43, 34, 20), 2)])
 def test_kernel_path_selection(k, grid, path):
     info = bte.bte_plan_info(W.config(k, grid=grid))
