@@ -320,3 +320,16 @@ def test_repeated_runs_are_bitwise_identical(bte, k, prec, warps, monkeypatch):
         if ref is None:
             ref = t.clone()
         assert bool((t == ref).all())
+
+
+@pytest.mark.parametrize("grid", [(1, 2, 2), (2, 4, 2), (1, 130, 36), (3, 66, 20), (7, 2, 34)])
+def test_fast_path_degenerate_extents(bte, grid):
+    """Fast path with fewer cells along x than the lane skew / the publication period, single-row tiles, and several
+    tiles in y and z at the same time (a unit finishes before its downstream tile may start)."""
+    p = W.config(4, grid=grid)
+    assert bte.Solver(p).kernel_path == 2
+    check(bte, p, 6, precision=W.FP64, checkpoints=(1, 2))
+    check(bte, p, 6, precision=W.FP32_STORE_FP64_ACC)
+    q = W.config(3, grid=grid)           # the same extents with the fin mask, periodic x, diffuse interfaces
+    if q.mask.sum() > 0:
+        check(bte, q, 6, precision=W.FP64, checkpoints=(1,))
