@@ -370,6 +370,7 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
       const int64_t na = a == 0 ? p->ny : p->nx, nb = a == 2 ? p->ny : p->nz;
       d.gf_off[f] = off; off += na * nb * B;
     }
+    d.gf_off[6] = off;
     pl.steps_total = (int64_t)pl.units2.size() * d.nsteps;
   }
   return BTE_OK;

@@ -77,7 +77,7 @@ struct Bte2Dev {
   double Pi_face[6];                // discrete hemispherical normaliser (reading G10)
   double wsa[BTE2_P][3];            // w_p |s_p,a|
   void *Gf;                         // T diffuse inflow [f][b][tb][ta]
-  int64_t gf_off[6];
+  int64_t gf_off[7];                // offsets of the 6 faces in Gf, [6] = total
   double *dT, *q, *qmag, *red;      // fp64 outputs in physical layout; residual partials
   int32_t n_red_blocks, pub_mask;   // progress is published when (t & pub_mask) == pub_mask
   int32_t slack, fill_iso;          // fill_iso: (re)write the constant isothermal ghost planes (first iteration only)
@@ -689,28 +689,32 @@ template <typename T>
 __global__ void bte2_gdiff_kernel(const __grid_constant__ Bte2Dev P) {
   constexpr int CP = 16 / sizeof(T), NCH = BTE2_P / CP;
   T *Gf = reinterpret_cast<T *>(P.Gf);
-  for (int f = 0; f < 6; ++f) {
+  // one flat index space over the entries of all six faces (all faces in flight at once)
+  for (int64_t eg = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; eg < P.gf_off[6]; eg += (int64_t)gridDim.x * blockDim.x) {
+    int f = 0;
+    while (f < 5 && eg >= P.gf_off[f + 1]) ++f;
     if (P.face_type[f] != 1) continue;
     const int a = f >> 1, side = f & 1;
     const Bte2Face g = bte2_face(P, a);
-    const int64_t nf = (int64_t)g.na * g.nb * P.B;
-    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < nf; e += (int64_t)gridDim.x * blockDim.x) {
-      const int ta = (int)(e % g.na), tb = (int)((e / g.na) % g.nb), b = (int)(e / ((int64_t)g.na * g.nb));
-      double H = 0.0;
-      for (int o = 0; o < 8; ++o) {
-        const Bte2Oct &O = P.oct[o];
-        const int sg = a == 0 ? O.sx : (a == 1 ? O.sy : O.sz);
-        if ((sg > 0) != (side == 1)) continue;          // outgoing octants only
-        int ip, jp, kp;
-        bte2_face_cell(P, o, a, side, ta, tb, ip, jp, kp);
-        for (int ch = 0; ch < NCH; ++ch) {
-          const Bte2Chunk<T> v = ldcg_chunk<T>(bte2_plane_chunk<T>(P, o, a, 1, b, ch, ip, jp, kp));
+    const int64_t e = eg - P.gf_off[f];
+    const int ta = (int)(e % g.na), tb = (int)((e / g.na) % g.nb), b = (int)(e / ((int64_t)g.na * g.nb));
+    double H = 0.0;
 #pragma unroll
-          for (int q = 0; q < CP; ++q) H += P.wsa[ch * CP + q][a] * (double)v.v[q];
-        }
-      }
-      Gf[P.gf_off[f] + e] = (T)(H / P.Pi_face[f]);
+    for (int o = 0; o < 8; ++o) {
+      const Bte2Oct &O = P.oct[o];
+      const int sg = a == 0 ? O.sx : (a == 1 ? O.sy : O.sz);
+      if ((sg > 0) != (side == 1)) continue;          // outgoing octants only
+      int ip, jp, kp;
+      bte2_face_cell(P, o, a, side, ta, tb, ip, jp, kp);
+      Bte2Chunk<T> v[NCH];
+#pragma unroll
+      for (int ch = 0; ch < NCH; ++ch) v[ch] = ldcg_chunk<T>(bte2_plane_chunk<T>(P, o, a, 1, b, ch, ip, jp, kp));
+#pragma unroll
+      for (int ch = 0; ch < NCH; ++ch)
+#pragma unroll
+        for (int q = 0; q < CP; ++q) H += P.wsa[ch * CP + q][a] * (double)v[ch].v[q];
     }
+    Gf[eg] = (T)(H / P.Pi_face[f]);
   }
 }
 
@@ -721,17 +725,24 @@ __global__ void bte2_ghost_kernel(const __grid_constant__ Bte2Dev P) {
   constexpr int CP = 16 / sizeof(T), NCH = BTE2_P / CP;
   const T *Gf = reinterpret_cast<const T *>(P.Gf);
   const int64_t gtid = blockIdx.x * (int64_t)blockDim.x + threadIdx.x, gstride = (int64_t)gridDim.x * blockDim.x;
-  for (int o = 0; o < 8; ++o) {
-    const Bte2Oct &O = P.oct[o];
-    for (int a = 0; a < 3; ++a) {
-      const int sg = a == 0 ? O.sx : (a == 1 ? O.sy : O.sz);
-      const int side = sg > 0 ? 0 : 1, f = 2 * a + side;   // physical face the octant enters through
-      const int type = P.face_type[f];
-      if (type >= 2) continue;      // specular / periodic: the sweep reads the lagged outflow buffer directly
-      if (type == 0 && !P.fill_iso) continue;   // isothermal planes are constant: written once
-      const Bte2Face g = bte2_face(P, a);
-      const int64_t n = (int64_t)g.na * g.nb * P.B * NCH;
-      for (int64_t e = gtid; e < n; e += gstride) {
+  // one flat index space over (octant, axis, plane entry)
+  const int64_t nseg[3] = {(int64_t)P.ny * P.nz * P.B * NCH, (int64_t)P.nx * P.nz * P.B * NCH, (int64_t)P.nx * P.ny * P.B * NCH};
+  const int64_t nper = nseg[0] + nseg[1] + nseg[2];
+  {
+    {
+      // (braces keep the historical indentation of the body)
+      for (int64_t eg = gtid; eg < 8 * nper; eg += gstride) {
+        const int o = (int)(eg / nper);
+        int64_t e = eg % nper;
+        int a = 0;
+        if (e >= nseg[0]) { e -= nseg[0]; a = 1; if (e >= nseg[1]) { e -= nseg[1]; a = 2; } }
+        const Bte2Oct &O = P.oct[o];
+        const int sg = a == 0 ? O.sx : (a == 1 ? O.sy : O.sz);
+        const int side = sg > 0 ? 0 : 1, f = 2 * a + side;   // physical face the octant enters through
+        const int type = P.face_type[f];
+        if (type >= 2) continue;      // specular / periodic: the sweep reads the lagged outflow buffer directly
+        if (type == 0 && !P.fill_iso) continue;   // isothermal planes are constant: written once
+        const Bte2Face g = bte2_face(P, a);
         // thread order follows the plane layouts so that writes coalesce: x planes [..][chunk][J]: j fastest;
         // y planes [..][i'][kk][chunk]: chunk, then i; z planes [..][u][jj][chunk][J]: j fastest, then chunk, then i
         int ta, tb, ch;
