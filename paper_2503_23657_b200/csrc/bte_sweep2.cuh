@@ -32,7 +32,6 @@
 #define BTE2_DIST(W, T) (((W) >= 8 && sizeof(T) == 4) ? 2 : 1)   // cp.async prefetch distance in steps (shared-memory budget)
 #define BTE2_MDIST(T) (sizeof(T) == 4 ? 1 : 0)   // same for the moment accumulator (fp64: fetched in the step that adds to it)
 #define BTE2_SLACK 0      // extra steps a unit lets the units it follows get ahead before it starts
-#define BTE2_TYROWS 64    // tile rows along y' (32 lanes x 2)
 
 template <typename T> struct alignas(16) Bte2Coefs {   // kernel parameter (constant bank 0)
   T k[BTE2_MAXB][8][BTE2_P];   // [band][inv, ax, ay, az, w/tau, v w|sx|, v w|sy|, v w|sz|][direction]
@@ -725,45 +724,40 @@ __global__ void bte2_ghost_kernel(const __grid_constant__ Bte2Dev P) {
   constexpr int CP = 16 / sizeof(T), NCH = BTE2_P / CP;
   const T *Gf = reinterpret_cast<const T *>(P.Gf);
   const int64_t gtid = blockIdx.x * (int64_t)blockDim.x + threadIdx.x, gstride = (int64_t)gridDim.x * blockDim.x;
-  // one flat index space over (octant, axis, plane entry)
+  // one flat index space over (octant, axis, plane entry): all planes are filled concurrently
   const int64_t nseg[3] = {(int64_t)P.ny * P.nz * P.B * NCH, (int64_t)P.nx * P.nz * P.B * NCH, (int64_t)P.nx * P.ny * P.B * NCH};
   const int64_t nper = nseg[0] + nseg[1] + nseg[2];
-  {
-    {
-      // (braces keep the historical indentation of the body)
-      for (int64_t eg = gtid; eg < 8 * nper; eg += gstride) {
-        const int o = (int)(eg / nper);
-        int64_t e = eg % nper;
-        int a = 0;
-        if (e >= nseg[0]) { e -= nseg[0]; a = 1; if (e >= nseg[1]) { e -= nseg[1]; a = 2; } }
-        const Bte2Oct &O = P.oct[o];
-        const int sg = a == 0 ? O.sx : (a == 1 ? O.sy : O.sz);
-        const int side = sg > 0 ? 0 : 1, f = 2 * a + side;   // physical face the octant enters through
-        const int type = P.face_type[f];
-        if (type >= 2) continue;      // specular / periodic: the sweep reads the lagged outflow buffer directly
-        if (type == 0 && !P.fill_iso) continue;   // isothermal planes are constant: written once
-        const Bte2Face g = bte2_face(P, a);
-        // thread order follows the plane layouts so that writes coalesce: x planes [..][chunk][J]: j fastest;
-        // y planes [..][i'][kk][chunk]: chunk, then i; z planes [..][u][jj][chunk][J]: j fastest, then chunk, then i
-        int ta, tb, ch;
-        if (a == 0) { ta = (int)(e % g.na); ch = (int)((e / g.na) % NCH); tb = (int)((e / ((int64_t)g.na * NCH)) % g.nb); }
-        else if (a == 1) { ch = (int)(e % NCH); ta = (int)((e / NCH) % g.na); tb = (int)((e / ((int64_t)g.na * NCH)) % g.nb); }
-        else { tb = (int)(e % g.nb); ch = (int)((e / g.nb) % NCH); ta = (int)((e / ((int64_t)g.nb * NCH)) % g.na); }
-        const int b = (int)(e / ((int64_t)g.na * NCH * g.nb));
-        int ip, jp, kp;
-        bte2_face_cell(P, o, a, side, ta, tb, ip, jp, kp);
-        Bte2Chunk<T> v;
-        if (type == 0) {
+  for (int64_t eg = gtid; eg < 8 * nper; eg += gstride) {
+    const int o = (int)(eg / nper);
+    int64_t e = eg % nper;
+    int a = 0;
+    if (e >= nseg[0]) { e -= nseg[0]; a = 1; if (e >= nseg[1]) { e -= nseg[1]; a = 2; } }
+    const Bte2Oct &O = P.oct[o];
+    const int sg = a == 0 ? O.sx : (a == 1 ? O.sy : O.sz);
+    const int side = sg > 0 ? 0 : 1, f = 2 * a + side;   // physical face the octant enters through
+    const int type = P.face_type[f];
+    if (type >= 2) continue;                  // specular / periodic: the sweep reads the lagged outflow buffer directly
+    if (type == 0 && !P.fill_iso) continue;   // isothermal planes are constant: written once
+    const Bte2Face g = bte2_face(P, a);
+    // thread order follows the plane layouts so that writes coalesce: x planes [..][chunk][J]: j fastest;
+    // y planes [..][i'][kk][chunk]: chunk, then i; z planes [..][u][jj][chunk][J]: j fastest, then chunk, then i
+    int ta, tb, ch;
+    if (a == 0) { ta = (int)(e % g.na); ch = (int)((e / g.na) % NCH); tb = (int)((e / ((int64_t)g.na * NCH)) % g.nb); }
+    else if (a == 1) { ch = (int)(e % NCH); ta = (int)((e / NCH) % g.na); tb = (int)((e / ((int64_t)g.na * NCH)) % g.nb); }
+    else { tb = (int)(e % g.nb); ch = (int)((e / g.nb) % NCH); ta = (int)((e / ((int64_t)g.nb * NCH)) % g.na); }
+    const int b = (int)(e / ((int64_t)g.na * NCH * g.nb));
+    int ip, jp, kp;
+    bte2_face_cell(P, o, a, side, ta, tb, ip, jp, kp);
+    Bte2Chunk<T> v;
+    if (type == 0) {
 #pragma unroll
-          for (int q = 0; q < CP; ++q) v.v[q] = (T)P.face_e0[f][b];
-        } else if (type == 1) {
-          const T gv = Gf[P.gf_off[f] + ((int64_t)b * g.nb + tb) * g.na + ta];
+      for (int q = 0; q < CP; ++q) v.v[q] = (T)P.face_e0[f][b];
+    } else {
+      const T gv = Gf[P.gf_off[f] + ((int64_t)b * g.nb + tb) * g.na + ta];
 #pragma unroll
-          for (int q = 0; q < CP; ++q) v.v[q] = gv;
-        }
-        *bte2_plane_chunk<T>(P, o, a, 0, b, ch, ip, jp, kp) = v;
-      }
+      for (int q = 0; q < CP; ++q) v.v[q] = gv;
     }
+    *bte2_plane_chunk<T>(P, o, a, 0, b, ch, ip, jp, kp) = v;
   }
   // interface faces: G = C dT_w / 4pi (isothermal) or (sum of the 4 outgoing octants' partial sums) / Pi_f (diffuse)
   T *Gi = reinterpret_cast<T *>(P.Gi);
