@@ -300,8 +300,8 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
   pl.v2 = v2;
   if (v2) {
     Bte2Dev &d = pl.d2;
-    int W = p->nz >= 48 ? 8 : 4;
-    if (const char *e = std::getenv("BTE_V2_W")) { const int w = std::atoi(e); if (w == 4 || w == 8) W = w; }
+    int W = p->nz >= 48 ? 8 : (p->nz <= 4 ? 2 : 4);   // 2 warps: thin slabs (the two-layer form of 2-D problems)
+    if (const char *e = std::getenv("BTE_V2_W")) { const int w = std::atoi(e); if (w == 2 || w == 4 || w == 8) W = w; }
     d.nx = p->nx; d.ny = p->ny; d.nz = p->nz; d.B = B; d.W = W;
     d.nty = (p->ny + 63) / 64; d.ntz = (p->nz + 2 * W - 1) / (2 * W); d.NU = p->nx + 31;
     d.nsteps = p->nx + 31 + W - 1;
@@ -613,7 +613,7 @@ bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t
     bte2_ghost_kernel<T><<<bgrid, 256, 0, st>>>(d);
     const bool tm = h->timing && h->ev_used + 2 <= h->ev.size();
     if (tm) CK(cudaEventRecord(h->ev[h->ev_used], st));
-    if (d.W == 8) launch_sweep2<T, 8>(h, cf, st); else launch_sweep2<T, 4>(h, cf, st);
+    if (d.W == 8) launch_sweep2<T, 8>(h, cf, st); else if (d.W == 4) launch_sweep2<T, 4>(h, cf, st); else launch_sweep2<T, 2>(h, cf, st);
     if (tm) { CK(cudaEventRecord(h->ev[h->ev_used + 1], st)); h->ev_used += 2; }
     bte2_update_kernel<T><<<pl.dev.n_red_blocks, 256, 0, st>>>(d);
     bte_final_kernel<<<1, 256, 0, st>>>(pl.dev);
@@ -642,7 +642,7 @@ bte_status setup_sweep2_W(bte_solver *h) {
 }
 template <typename T>
 bte_status setup_sweep2(bte_solver *h) {
-  return h->pl.d2.W == 8 ? setup_sweep2_W<T, 8>(h) : setup_sweep2_W<T, 4>(h);
+  return h->pl.d2.W == 8 ? setup_sweep2_W<T, 8>(h) : (h->pl.d2.W == 4 ? setup_sweep2_W<T, 4>(h) : setup_sweep2_W<T, 2>(h));
 }
 
 template <typename T>

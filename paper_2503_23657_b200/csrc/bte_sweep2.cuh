@@ -489,6 +489,9 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     const bool slowmask = MASKED && __any_sync(FULL, live && !plain);
     const Ch *__restrict__ zrd = K == 0 ? &S->zin0[rb][0][0][J] : &S->zex[cur][K - 1][0][0][J];
     Ch *__restrict__ zwr = &S->zex[cur ^ 1][K][0][0][J];
+    // warps without a valid row (ragged last z tile; 3 of 4 warps of a two-layer 2-D slab) and warps that are
+    // entirely before their first or after their last cell skip the arithmetic (they still stage and synchronise)
+    if (__any_sync(FULL, act))
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
       V2 r[2][2];
