@@ -30,7 +30,7 @@ const double kFourPi = 12.566370614359172953850573533118;
 struct Plan {
   BteDev dev{};                          // geometry part filled by build_plan, pointers by carve()
   std::vector<uint8_t> code;             // [ncell]
-  std::vector<int32_t> iface, iface_info;
+  std::vector<int32_t> iface, iface_info, iface_cell;
   std::vector<double> Q;                 // [ncell]
   std::vector<double> band;              // [4][B]
   std::vector<double> coef;              // unique coefficient blocks, 16x8 doubles each
@@ -135,6 +135,7 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
         pl.code[c] |= (uint8_t)(2 << f);
         iface[(size_t)f * N + c] = nif++;
         pl.iface_info.push_back(f);
+        pl.iface_cell.push_back((int32_t)c);
       }
     }
   }
@@ -343,7 +344,7 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
       U.b0 = g * NBmax; U.nb = std::min(NBmax, B - U.b0);
     }
     d.n_iface = nif; d.iface_type = p->interface_bc.type;
-    for (int b = 0; b < B; ++b) { d.iface_e0[b] = pl.band[b] * p->interface_bc.dT_wall; d.vband[b] = p->v[b]; }
+    for (int b = 0; b < B; ++b) { d.iface_e0[b] = pl.band[b] * p->interface_bc.dT_wall; d.ivband[b] = 1.0 / p->v[b]; }
     if (pl.masked2) {
       const size_t NPp = (size_t)(p->nz / 2) * d.nty * d.NU * 32;
       for (int cl = 0; cl < 4; ++cl) {
@@ -426,13 +427,14 @@ size_t bind(Plan &pl, unsigned char *ws) {
       for (int c = 0; c < 4; ++c) d.codeP[c] = (const uint32_t *)take((size_t)(dv.nz / 2) * d.nty * d.NU * 32 * 4);
       d.iface = d.n_iface ? (const int32_t *)take((size_t)6 * N * 4) : nullptr;
       d.iface_info = d.n_iface ? (const int32_t *)take((size_t)d.n_iface * 4) : nullptr;
+      d.iface_cell = d.n_iface ? (const int32_t *)take((size_t)d.n_iface * 4) : nullptr;
     } else {
-      d.code = nullptr; d.iface = nullptr; d.iface_info = nullptr;
+      d.code = nullptr; d.iface = nullptr; d.iface_info = nullptr; d.iface_cell = nullptr;
       for (int c = 0; c < 4; ++c) d.codeP[c] = nullptr;
     }
     pl.state_begin = off;
     d.Gi = d.n_iface ? take((size_t)d.n_iface * d.B * tsz) : nullptr;
-    d.Hpart = d.n_iface ? (double *)take((size_t)d.n_iface * d.B * 4 * 8) : nullptr;
+    d.Hd = (d.n_iface && d.iface_type == 1) ? take((size_t)6 * N * d.B * 4 * tsz) : nullptr;
     d.prog = (int32_t *)take((size_t)d.n_units * 4);
     d.ticket = (int32_t *)take(256);
     dv.red = (double *)take((size_t)(4 * dv.n_red_blocks + 4) * 8);
@@ -722,6 +724,7 @@ bte_status bte_create(const bte_problem *p, void *d_workspace, size_t bytes, voi
       if (pl.d2.n_iface) {
         CKD(cudaMemcpyAsync((void *)pl.d2.iface, pl.iface.data(), pl.iface.size() * 4, cudaMemcpyHostToDevice, s));
         CKD(cudaMemcpyAsync((void *)pl.d2.iface_info, pl.iface_info.data(), pl.iface_info.size() * 4, cudaMemcpyHostToDevice, s));
+        CKD(cudaMemcpyAsync((void *)pl.d2.iface_cell, pl.iface_cell.data(), pl.iface_cell.size() * 4, cudaMemcpyHostToDevice, s));
       }
     }
   } else {

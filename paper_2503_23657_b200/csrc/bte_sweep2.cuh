@@ -90,10 +90,12 @@ struct Bte2Dev {
   const int32_t *iface;             // [6][ncell] interface-face id or -1
   const int32_t *iface_info;        // [n_iface] face code f
   void *Gi;                         // T [n_iface][B] interface inflow of this iteration (Eq. 5 / Eq. 6)
-  double *Hpart;                    // [n_iface][B][4] outgoing hemispherical partial sums per octant slot
+  void *Hd;                         // T [6][ncell][B][4] outgoing hemispherical partial sums per face, cell, band and
+                                    // outgoing-octant slot (dense, touched at interface faces only: no id look-up in the sweep)
+  const int32_t *iface_cell;        // [n_iface] physical cell of the face
   int32_t n_iface, iface_type;
   double iface_e0[BTE2_MAXB];       // isothermal interface inflow C_b dT_w / 4pi
-  double vband[BTE2_MAXB];          // group velocities (to undo the v_b in the moment coefficients)
+  double ivband[BTE2_MAXB];         // 1 / group velocity (undoes the v_b in the moment coefficients)
 };
 
 // ------------------------------------------------------------------ layouts (host + device)
@@ -516,7 +518,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
           for (int a = 0; a < 3; ++a) {
             g[cc][a] = (T)0;
             if (live && (cb[cc] & 1u) && ((cb[cc] >> (1 + fu[a])) & 1u))
-              g[cc][a] = P.iface_type == 0 ? (T)P.iface_e0[b0 + b]
+              g[cc][a] = (P.iface_type == 0 || (P.dbg & 64)) ? (T)P.iface_e0[b0 + b]
                                            : reinterpret_cast<const T *>(P.Gi)[(int64_t)__ldg(P.iface + (int64_t)fu[a] * P.ncell + cph[cc]) * P.B + b0 + b];
           }
         }
@@ -528,7 +530,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
 #pragma unroll
           for (int cc = 0; cc < 4; ++cc)
             if (cb[cc] & 1u) anydn |= cb[cc] & ((2u << (fu[0] ^ 1)) | (2u << (fu[1] ^ 1)) | (2u << (fu[2] ^ 1)));
-          if (P.iface_type == 1 && live && anydn != 0) {
+          if (P.iface_type == 1 && live && anydn != 0 && !(P.dbg & 128)) {
 #pragma unroll
             for (int cc = 0; cc < 4; ++cc) {
               const int jj = cc & 1, kk = cc >> 1;
@@ -543,11 +545,9 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
 #pragma unroll
                 for (int q = 0; q < BTE2_P / 2; ++q)
                   hs = fma2(mk2(CF.k[b0 + b][5 + a][2 * q], CF.k[b0 + b][5 + a][2 * q + 1]), c[jj][kk][b * (BTE2_P / 2) + q], hs);
-                const double hsum = ((double)hs.x + (double)hs.y) / P.vband[b0 + b];
                 const int bx = O.sx < 0, by = O.sy < 0, bz = O.sz < 0;
                 const int s2 = a == 0 ? (by | (bz << 1)) : (a == 1 ? (bx | (bz << 1)) : (bx | (by << 1)));
-                const int64_t fid = P.iface[(int64_t)fd * P.ncell + cph[cc]];
-                P.Hpart[(fid * P.B + b0 + b) * 4 + s2] = hsum;
+                reinterpret_cast<T *>(P.Hd)[(((int64_t)fd * P.ncell + cph[cc]) * P.B + b0 + b) * 4 + s2] = (hs.x + hs.y) * (T)P.ivband[b0 + b];
               }
             }
           }
@@ -770,7 +770,8 @@ __global__ void bte2_ghost_kernel(const __grid_constant__ Bte2Dev P) {
     const int b = (int)(e % P.B);
     if (P.iface_type == 0) { Gi[e] = (T)P.iface_e0[b]; continue; }
     double H = 0.0;
-    for (int sl = 0; sl < 4; ++sl) H += P.Hpart[e * 4 + sl];
+    const T *hp = reinterpret_cast<const T *>(P.Hd) + (((int64_t)P.iface_info[fid] * P.ncell + P.iface_cell[fid]) * P.B + b) * 4;
+    for (int sl = 0; sl < 4; ++sl) H += (double)hp[sl];
     Gi[e] = (T)(H / P.Pi_face[P.iface_info[fid]]);
   }
   if (gtid == 0) *P.ticket = 0;
