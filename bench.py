@@ -212,7 +212,9 @@ def run_ours(args, W):
 
     # ---- end to end through the C-ABI host-buffer call: every step uploads Q from pinned host memory,
     # runs one iteration and downloads dT into pinned host memory
-    Qh = torch.from_numpy(p.Q.astype("float64")).contiguous().pin_memory()
+    import numpy as np
+    Qsrc = p.Q if p.Q is not None else np.zeros((p.nz, p.ny, p.nx))
+    Qh = torch.from_numpy(np.ascontiguousarray(Qsrc, dtype=np.float64)).pin_memory()
     dTh = torch.empty(solver.shape, dtype=torch.float64).pin_memory()
     for _ in range(3):
         solver.solve_host(Qh, 1, reset=False, out=(dTh, None))

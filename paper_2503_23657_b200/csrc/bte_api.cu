@@ -591,6 +591,19 @@ bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t
     if (ep == 1 && h->iters > 0) CK(cudaMemsetAsync(d.prog, 0, (size_t)d.n_units * 4, st));
     d.epoch = ep;
     d.fill_iso = h->iters == 0;
+    {   // ghost planes to fill: diffuse faces every iteration, isothermal faces once (specular / periodic: none)
+      const int NCHh = (int)(BTE2_P * (pl.dev.fp32 ? 4 : 8) / 16);
+      const int64_t nseg[3] = {(int64_t)d.ny * d.nz * d.B * NCHh, (int64_t)d.nx * d.nz * d.B * NCHh, (int64_t)d.nx * d.ny * d.B * NCHh};
+      d.gseg_n = 0; d.gseg_off[0] = 0;
+      for (int o = 0; o < 8; ++o) for (int a = 0; a < 3; ++a) {
+        const int sg = a == 0 ? d.oct[o].sx : (a == 1 ? d.oct[o].sy : d.oct[o].sz);
+        const int type = d.face_type[2 * a + (sg > 0 ? 0 : 1)];
+        if (type >= 2 || (type == 0 && !d.fill_iso)) continue;
+        d.gseg_oa[d.gseg_n] = o * 3 + a;
+        d.gseg_off[d.gseg_n + 1] = d.gseg_off[d.gseg_n] + nseg[a];
+        ++d.gseg_n;
+      }
+    }
     {   // inflow sources / outflow buffers of this iteration (parity of the epoch)
       const size_t cur = (size_t)(ep & 1), prev = cur ^ 1;
       auto xo = [&](int o, size_t par) { return (char *)d.oct[o].xout + par * pl.x2_chunks * 16; };

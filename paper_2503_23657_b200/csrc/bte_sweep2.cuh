@@ -80,6 +80,9 @@ struct Bte2Dev {
   double *dT, *q, *qmag, *red;      // fp64 outputs in physical layout; residual partials
   int32_t n_red_blocks, pub_mask;   // progress is published when (t & pub_mask) == pub_mask
   int32_t slack, fill_iso;          // fill_iso: (re)write the constant isothermal ghost planes (first iteration only)
+  // ghost planes to fill in this iteration: (octant, axis) segments and their offsets in one flat index space
+  int32_t gseg_n, gseg_oa[24];
+  int64_t gseg_off[25];
   int64_t ncell, src_mod;            // src_mod: cells of the caller's field (2-D problems run as two layers)
   double inv_sumCtau;
   // voxel masks (all null / 0 when every cell is solid).  Cell byte: bit0 solid, bit 1+f: the neighbour across
@@ -727,20 +730,16 @@ __global__ void bte2_ghost_kernel(const __grid_constant__ Bte2Dev P) {
   constexpr int CP = 16 / sizeof(T), NCH = BTE2_P / CP;
   const T *Gf = reinterpret_cast<const T *>(P.Gf);
   const int64_t gtid = blockIdx.x * (int64_t)blockDim.x + threadIdx.x, gstride = (int64_t)gridDim.x * blockDim.x;
-  // one flat index space over (octant, axis, plane entry): all planes are filled concurrently
-  const int64_t nseg[3] = {(int64_t)P.ny * P.nz * P.B * NCH, (int64_t)P.nx * P.nz * P.B * NCH, (int64_t)P.nx * P.ny * P.B * NCH};
-  const int64_t nper = nseg[0] + nseg[1] + nseg[2];
-  for (int64_t eg = gtid; eg < 8 * nper; eg += gstride) {
-    const int o = (int)(eg / nper);
-    int64_t e = eg % nper;
-    int a = 0;
-    if (e >= nseg[0]) { e -= nseg[0]; a = 1; if (e >= nseg[1]) { e -= nseg[1]; a = 2; } }
+  // one flat index space over the (octant, axis) ghost planes that need filling: all of them concurrently
+  for (int64_t eg = gtid; eg < P.gseg_off[P.gseg_n]; eg += gstride) {
+    int sgi = 0;
+    while (sgi + 1 < P.gseg_n && eg >= P.gseg_off[sgi + 1]) ++sgi;
+    const int o = P.gseg_oa[sgi] / 3, a = P.gseg_oa[sgi] % 3;
+    const int64_t e = eg - P.gseg_off[sgi];
     const Bte2Oct &O = P.oct[o];
     const int sg = a == 0 ? O.sx : (a == 1 ? O.sy : O.sz);
     const int side = sg > 0 ? 0 : 1, f = 2 * a + side;   // physical face the octant enters through
-    const int type = P.face_type[f];
-    if (type >= 2) continue;                  // specular / periodic: the sweep reads the lagged outflow buffer directly
-    if (type == 0 && !P.fill_iso) continue;   // isothermal planes are constant: written once
+    const int type = P.face_type[f];                     // 0 isothermal (Eq. 5) or 1 diffuse (Eq. 6)
     const Bte2Face g = bte2_face(P, a);
     // thread order follows the plane layouts so that writes coalesce: x planes [..][chunk][J]: j fastest;
     // y planes [..][i'][kk][chunk]: chunk, then i; z planes [..][u][jj][chunk][J]: j fastest, then chunk, then i
