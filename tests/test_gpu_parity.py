@@ -268,10 +268,11 @@ def test_config3_full(bte):
 
 @pytest.mark.slow
 def test_config4_full_sampled(bte):
-    """Full-size config 4 in the launch configuration bench.py times: 2 iterations against the
-    (multi-threaded, bit-identical) oracle on every cell, plus size-independent properties."""
+    """Full-size config 4 in the launch configuration bench.py times: n = 5 iterations against the
+    (multi-threaded, bit-identical) oracle on every cell; the converged state is checked by
+    test_config4_full_converged_energy_balance and, like for like, by test_config4_replica_converged_state."""
     p = W.config(4)
-    out = check(bte, p, 2, checkpoints=(1,))
+    out = check(bte, p, 5, checkpoints=(1, 2))
     assert out[-1][1] <= 1e-4
 
 
