@@ -306,7 +306,9 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
     d.nx = p->nx; d.ny = p->ny; d.nz = p->nz; d.B = B; d.W = W;
     d.nty = (p->ny + 63) / 64; d.ntz = (p->nz + 2 * W - 1) / (2 * W); d.NU = p->nx + 31;
     d.nsteps = p->nx + 31 + W - 1;
-    if (const char *e = std::getenv("BTE_V2_DBG")) d.dbg = std::atoi(e);
+#ifdef BTE2_ENABLE_DBG
+    if (const char *e = std::getenv("BTE_V2_DBG")) d.dbg = std::atoi(e);   // timing experiments (skips parts of the kernel)
+#endif
     d.pub_mask = BTE2_PUB - 1; d.slack = BTE2_SLACK;
     if (const char *e = std::getenv("BTE_V2_PUB")) { const int v = std::atoi(e); if (v == 4 || v == 8 || v == 16 || v == 32) d.pub_mask = v - 1; }
     if (const char *e = std::getenv("BTE_V2_SLACK")) { const int v = std::atoi(e); if (v >= 0 && v <= 256) d.slack = v; }

@@ -32,6 +32,12 @@
 #define BTE2_DIST(W, T) (((W) >= 8 && sizeof(T) == 4) ? 2 : 1)   // cp.async prefetch distance in steps (shared-memory budget)
 #define BTE2_MDIST(T) (sizeof(T) == 4 ? 1 : 0)   // same for the moment accumulator (fp64: fetched in the step that adds to it)
 #define BTE2_SLACK 0      // extra steps a unit lets the units it follows get ahead before it starts
+// timing experiments only (-DBTE2_ENABLE_DBG + env BTE_V2_DBG): the product build compiles the switches out
+#ifdef BTE2_ENABLE_DBG
+#define BTE2_DBGBIT(P, bit) ((P).dbg & (bit))
+#else
+#define BTE2_DBGBIT(P, bit) 0
+#endif
 
 template <typename T> struct alignas(16) Bte2Coefs {   // kernel parameter (constant bank 0)
   T k[BTE2_MAXB][8][BTE2_P];   // [band][inv, ax, ay, az, w/tau, v w|sx|, v w|sy|, v w|sz|][direction]
@@ -143,8 +149,7 @@ __device__ __forceinline__ void st_release_gpu(int *p, int v) {
   asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 template <int BYTES>
-__device__ __forceinline__ void cp_async(void *smem_dst, const void *gsrc) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+__device__ __forceinline__ void cp_async(unsigned d, const void *gsrc) {   // d: shared-window address
   if (BYTES == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
   else if (BYTES == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
   else if (BYTES == 4) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
@@ -214,6 +219,8 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
   const int Jl = (min(P.ny, (ty + 1) * 64) - 1 - ty * 64) >> 1, Kl = (min(P.nz, (tz + 1) * 2 * W) - 1 - tz * 2 * W) >> 1;
   const bool first = un.dep_prev < 0;                  // first band group of this octant: M is written, not added to
   const int ebase = P.epoch << 16;
+  // shared-window address for cp.async (hoisting one base address out of the step loop measured slower in fp32)
+  auto saddr = [&](const void *ptr) { return (unsigned)__cvta_generic_to_shared(ptr); };
 
   const Ch *xin = reinterpret_cast<const Ch *>(O.xsrc);
   Ch *xout = reinterpret_cast<Ch *>(O.xdst);
@@ -253,7 +260,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
   const int mylag = tid == 0 ? 33 : (tid == 1 ? W + 1 : 1);
   int seen = 0, peek = 0;
   auto ensure = [&](int t1) {          // everything step t1 reads from other units has been published
-    if (mydep >= 0 && !(P.dbg & 4)) {
+    if (mydep >= 0 && !BTE2_DBGBIT(P, 4)) {
       seen = max(seen, peek - ebase);
       if (seen < t1 + mylag) {
         int v;
@@ -266,7 +273,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
   // ---- previous content of the moment accumulator for step t1 (own commit group, one step ahead)
   auto prefetch_m = [&](int t1) {
     const int ip1 = t1 - J - K;
-    if (!first && !(P.dbg & 2) && vthread && ip1 >= 0 && ip1 < P.nx) {
+    if (!first && !BTE2_DBGBIT(P, 2) && vthread && ip1 >= 0 && ip1 < P.nx) {
 #pragma unroll
       for (int kk = 0; kk < 2; ++kk)
 #pragma unroll
@@ -274,19 +281,19 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
           const int64_t ci = cbase[kk] + jj * 32 + (int64_t)t1 * 64;
 #pragma unroll
           for (int h = 0; h < (int)sizeof(Bte2Mom<T>) / 16; ++h)
-            cp_async<16>(reinterpret_cast<char *>(&S->mold[t1 % (BTE2_MDIST(T) + 1)][kk][jj][tid]) + 16 * h, reinterpret_cast<const char *>(M + ci) + 16 * h);
+            cp_async<16>(saddr(&S->mold[t1 % (BTE2_MDIST(T) + 1)][kk][jj][tid]) + 16 * h, reinterpret_cast<const char *>(M + ci) + 16 * h);
         }
     }
   };
   // ---- outflow faces of step t1 (staged in shared memory by the step) -> global planes, coalesced
   auto copy_out = [&](int t1) {
     const int par = (t1 & 1) ^ 1;                      // buffer the step wrote
-    if (!(P.dbg & 1) && kp0 < P.nz) {
+    if (!BTE2_DBGBIT(P, 1) && kp0 < P.nz) {
       const int ipl = t1 - Jl - K;                     // cell lane Jl of this warp finished in step t1
       if (J < 2 * NC && ipl >= 0 && ipl < P.nx) ydst[(int64_t)ipl * 2 * NCH] = S->yst[par][K][ykk * NC + yb * NCH + ych];
     }
     const int ul = t1 - Kl;
-    if (!(P.dbg & 1) && ul >= 0 && ul < P.NU) {
+    if (!BTE2_DBGBIT(P, 1) && ul >= 0 && ul < P.NU) {
 #pragma unroll
       for (int q = 0; q < (2 * NC * 32) / NT; ++q) {
         const int e = tid + q * NT, b = e / (2 * NCH * 32), rem = e % (2 * NCH * 32);
@@ -295,8 +302,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     }
   };
   // ---- asynchronous prefetch (global -> shared) of everything step t1 consumes
-  auto prefetch = [&](int t1) {
-    const int rb = t1 % R;
+  auto prefetch = [&](int t1, int rb) {                // rb = t1 % R, the ring slot of step t1
     const int ip1 = t1 - J - K;
     if (vthread && ip1 >= 0 && ip1 < P.nx) {
 #pragma unroll
@@ -304,21 +310,21 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
 #pragma unroll
           for (int jj = 0; jj < 2; ++jj) {
             const int64_t ci = cbase[kk] + jj * 32 + (int64_t)t1 * 64;
-            cp_async<sizeof(Bte2Pair<T>)>(&S->inp[rb][kk][jj][tid], dTQ + ci);
+            cp_async<sizeof(Bte2Pair<T>)>(saddr(&S->inp[rb][kk][jj][tid]), dTQ + ci);
           }
         }
     }
-    if (MASKED && vthread && ip1 >= 0 && ip1 < P.nx) cp_async<4>(&S->codes[rb][tid], cpsrc + (int64_t)t1 * 32);
-    if (t1 < P.NU && !(P.dbg & 8)) {
+    if (MASKED && vthread && ip1 >= 0 && ip1 < P.nx) cp_async<4>(saddr(&S->codes[rb][tid]), cpsrc + (int64_t)t1 * 32);
+    if (t1 < P.NU && !BTE2_DBGBIT(P, 8)) {
 #pragma unroll
       for (int q = 0; q < (2 * NC * 32) / NT; ++q) {
         const int e = tid + q * NT, b = e / (2 * NCH * 32), rem = e % (2 * NCH * 32);
-        cp_async<16>(&S->zin0[rb][0][b * NCH][0] + (rem / (NCH * 32)) * (NC * 32) + (rem % (NCH * 32)), zsrc + b * zband + t1 * zstep + rem);
+        cp_async<16>(saddr(&S->zin0[rb][0][b * NCH][0] + (rem / (NCH * 32)) * (NC * 32) + (rem % (NCH * 32))), zsrc + b * zband + t1 * zstep + rem);
       }
     }
     {
       const int ipy = t1 - K;
-      if (J < 2 * NC && ipy >= 0 && ipy < P.nx) cp_async<16>(&S->ybuf[rb][K][ykk][yb * NCH + ych], ysrc + (int64_t)t1 * 2 * NCH);
+      if (J < 2 * NC && ipy >= 0 && ipy < P.nx) cp_async<16>(saddr(&S->ybuf[rb][K][ykk][yb * NCH + ych]), ysrc + (int64_t)t1 * 2 * NCH);
     }
   };
 
@@ -343,7 +349,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
 #pragma unroll
   for (int t1 = 0; t1 < D; ++t1) {
     if (t1 == 0 && BTE2_MDIST(T) == 1) prefetch_m(0);
-    prefetch(t1); cp_async_commit();
+    prefetch(t1, t1); cp_async_commit();
   }
   cp_async_wait<D - 1>();
   __syncthreads();
@@ -452,13 +458,14 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     zwr[cn * 32] = o0; zwr[(NC + cn) * 32] = o1;
   };
 
+  int rb = 0, rbp = R - 1;                             // ring slots of step t and of step t - 1 (= step t + D)
   for (int t = 0; t < P.nsteps; ++t) {
-    const int cur = t & 1, rb = t % R;
+    const int cur = t & 1;
     const int ip = t - J - K;
     const bool act = vthread && ip >= 0 && ip < P.nx;
     prefetch_m(t + BTE2_MDIST(T));
     cp_async_commit();
-    prefetch(t + D);
+    prefetch(t + D, rbp);
     cp_async_commit();
     if (t > 0) copy_out(t - 1);
     if (tid < 3 && mydep >= 0 && seen < t + 1 + D + mylag) peek = ld_acquire_gpu(P.prog + mydep);   // consumed by ensure() below
@@ -521,7 +528,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
           for (int a = 0; a < 3; ++a) {
             g[cc][a] = (T)0;
             if (live && (cb[cc] & 1u) && ((cb[cc] >> (1 + fu[a])) & 1u))
-              g[cc][a] = (P.iface_type == 0 || (P.dbg & 64)) ? (T)P.iface_e0[b0 + b]
+              g[cc][a] = (P.iface_type == 0 || BTE2_DBGBIT(P, 64)) ? (T)P.iface_e0[b0 + b]
                                            : reinterpret_cast<const T *>(P.Gi)[(int64_t)__ldg(P.iface + (int64_t)fu[a] * P.ncell + cph[cc]) * P.B + b0 + b];
           }
         }
@@ -533,7 +540,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
 #pragma unroll
           for (int cc = 0; cc < 4; ++cc)
             if (cb[cc] & 1u) anydn |= cb[cc] & ((2u << (fu[0] ^ 1)) | (2u << (fu[1] ^ 1)) | (2u << (fu[2] ^ 1)));
-          if (P.iface_type == 1 && live && anydn != 0 && !(P.dbg & 128)) {
+          if (P.iface_type == 1 && live && anydn != 0 && !BTE2_DBGBIT(P, 128)) {
 #pragma unroll
             for (int cc = 0; cc < 4; ++cc) {
               const int jj = cc & 1, kk = cc >> 1;
@@ -569,7 +576,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
       // (b) moments of this band group into the octant accumulator (one owner per cell and group)
 #pragma unroll
       for (int kk = 0; kk < 2; ++kk)
-        if (!(P.dbg & 2)) {
+        if (!BTE2_DBGBIT(P, 2)) {
 #pragma unroll
           for (int jj = 0; jj < 2; ++jj) {
             if (MASKED && !(cb[jj + 2 * kk] & 1u)) continue;      // void cell
@@ -610,6 +617,8 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
       __threadfence();
       st_release_gpu(P.prog + unit, ebase + t);
     }
+    rbp = rb;
+    rb = rb + 1 == R ? 0 : rb + 1;
   }
   cp_async_wait<0>();
   copy_out(P.nsteps - 1);
