@@ -165,10 +165,8 @@ template <typename T> __device__ __forceinline__ Bte2Chunk<T> ldcg_chunk(const B
 }
 // packed pairs of directions: fp32 uses the sm_100 two-wide FMA (FFMA2: two FMAs per issue slot, which frees
 // issue slots for the non-FMA instructions of the step); fp64 is two scalar DFMAs.
-// Measured on B200 (_work microbenchmarks): FFMA2 whose coefficient operand is a PAIR of
-// uniform registers runs at half the FMA rate (64 FMA/clk/SM); with a broadcast scalar uniform register or
-// vector-register operands it runs at full rate, but those forms cost pair-assembly moves or 16 more registers
-// here (both tried, both slower in this kernel).
+// Measured on B200 (csrc/microbench_fma_forms.cu, profiles/r01_fma_forms_microbench.txt): FFMA2 with two vector-register
+// operands and a uniform-register pair (the form used here) runs at the full FMA rate, 124.6 of 128 FMA/clk/SM.
 template <typename T> struct Bte2V2;
 template <> struct Bte2V2<float> { typedef float2 t; };
 template <> struct Bte2V2<double> { typedef double2 t; };
