@@ -549,10 +549,14 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
                 if (!((cb[cc] >> (1 + fd)) & 1u)) continue;
                 // sum_p w_p |s_p,a| e_p in the compute type with the moment coefficients v_b w |s_a| (<= 16 terms of
                 // one sign pattern), divided by v_b; the sum over the 4 outgoing octants is fp64 (ghost kernel)
+                // The first band of the group gets it for free: it IS the cell's first-moment partial sum so far.
                 V2 hs = mk2((T)0, (T)0);
+                if (b == 0) hs = m[jj][kk][1 + a];
+                else {
 #pragma unroll
-                for (int q = 0; q < BTE2_P / 2; ++q)
-                  hs = fma2(mk2(CF.k[b0 + b][5 + a][2 * q], CF.k[b0 + b][5 + a][2 * q + 1]), c[jj][kk][b * (BTE2_P / 2) + q], hs);
+                  for (int q = 0; q < BTE2_P / 2; ++q)
+                    hs = fma2(mk2(CF.k[b0 + b][5 + a][2 * q], CF.k[b0 + b][5 + a][2 * q + 1]), c[jj][kk][b * (BTE2_P / 2) + q], hs);
+                }
                 const int bx = O.sx < 0, by = O.sy < 0, bz = O.sz < 0;
                 const int s2 = a == 0 ? (by | (bz << 1)) : (a == 1 ? (bx | (bz << 1)) : (bx | (by << 1)));
                 reinterpret_cast<T *>(P.Hd)[(((int64_t)fd * P.ncell + cph[cc]) * P.B + b0 + b) * 4 + s2] = (hs.x + hs.y) * (T)P.ivband[b0 + b];
