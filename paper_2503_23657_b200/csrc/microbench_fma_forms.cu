@@ -35,6 +35,33 @@ __global__ void __launch_bounds__(256) kern(const __grid_constant__ Coefs CF, fl
   for (int i = 0; i < NACC; ++i) s += a[i].x + a[i].y;
   out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
+
+// dependent-issue latency: ONE warp per SM, one accumulator chain (each instruction needs the previous result)
+template <int FORM>
+__global__ void __launch_bounds__(32) lat(const __grid_constant__ Coefs CF, float *out, const float *vin, long long *cyc) {
+  float2 a = make_float2(threadIdx.x * 1e-3f, 0.5f);
+  const float2 v = make_float2(vin[threadIdx.x & 63], vin[(threadIdx.x + 1) & 63]);
+  const long long t0 = clock64();
+  for (int it = 0; it < ITERS; ++it) {
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+      if (FORM == 0) a.x = fmaf(a.x, CF.k[j], v.y);                                        // FFMA R,UR,R chain
+      if (FORM == 1) a = __ffma2_rn(a, make_float2(CF.k[2 * (j & 7)], CF.k[2 * (j & 7) + 1]), v);   // FFMA2 R,URpair,R chain
+      if (FORM == 2) a = __ffma2_rn(v, make_float2(CF.k[2 * (j & 7)], CF.k[2 * (j & 7) + 1]), a);   // FFMA2 accumulate chain
+    }
+  }
+  const long long t1 = clock64();
+  out[blockIdx.x * 32 + threadIdx.x] = a.x + a.y;
+  if (threadIdx.x == 0 && blockIdx.x == 0) *cyc = t1 - t0;
+}
+template <int FORM> void runlat(const char *name, float *out, float *vin) {
+  Coefs cf; for (int i = 0; i < 64; ++i) cf.k[i] = 0.5f + 1e-3f * i;
+  long long *d, h = 0; cudaMalloc(&d, 8);
+  lat<FORM><<<148, 32>>>(cf, out, vin, d); cudaDeviceSynchronize();
+  cudaMemcpy(&h, d, 8, cudaMemcpyDeviceToHost);
+  printf("%-28s dependent chain: %.2f cycles per instruction\n", name, (double)h / (ITERS * 32.0));
+  cudaFree(d);
+}
 template <int FORM> void run(const char *name, int blocks_per_sm, float *out, float *vin) {
   Coefs cf; for (int i = 0; i < 64; ++i) cf.k[i] = 0.5f + 1e-3f * i;
   cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
@@ -59,5 +86,8 @@ int main() {
     run<6>("FFMA  acc+=R*UR", bps, out, vin);
     run<7>("FFMA2 acc+=R*URbcast", bps, out, vin);
   }
+  runlat<0>("FFMA  R,UR,R", out, vin);
+  runlat<1>("FFMA2 R,URpair,R", out, vin);
+  runlat<2>("FFMA2 acc+=R*URpair", out, vin);
   return 0;
 }
