@@ -365,6 +365,9 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     if (t1 == 0 && BTE2_MDIST(T) == 1) prefetch_m(0);
     prefetch(t1, t1); cp_async_commit();
   }
+#if BTE2_SPLITBAR
+  prefetch_m(BTE2_MDIST(T)); cp_async_commit();        // steady state: issued in the barrier window of the previous step
+#endif
   cp_async_wait<D - 1>();
   __syncthreads();
 
@@ -477,8 +480,10 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     const int cur = t & 1;
     const int ip = t - J - K;
     const bool act = vthread && ip >= 0 && ip < P.nx;
+#if !BTE2_SPLITBAR
     prefetch_m(t + BTE2_MDIST(T));
     cp_async_commit();
+#endif
     prefetch(t + D, rbp);
     cp_async_commit();
     if (t > 0) copy_out(t - 1);
@@ -634,6 +639,10 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
       }
     }
 #if BTE2_SPLITBAR
+    // accumulator rows of the step after next: their publication upstream is known since the previous barrier
+    // (ensure(t + D) covers step t + 1 + MDIST because D >= 1 + MDIST), and the ring slot was read just above
+    prefetch_m(t + 1 + BTE2_MDIST(T));
+    cp_async_commit();
     mbar_wait(stepbar, bpar);          // every thread has arrived: the moment store above overlapped the wait
     bpar ^= 1u;
     __syncwarp();                      // yst rows written after the arrive are read by this warp's copy_out next step
