@@ -62,6 +62,36 @@ template <int FORM> void runlat(const char *name, float *out, float *vin) {
   printf("%-28s dependent chain: %.2f cycles per instruction\n", name, (double)h / (ITERS * 32.0));
   cudaFree(d);
 }
+
+// FP64: DFMA throughput (register operands), same launch shape
+__global__ void __launch_bounds__(256) kern64(double *out, const double *vin) {
+  double a[NACC];
+#pragma unroll
+  for (int i = 0; i < NACC; ++i) a[i] = threadIdx.x * 1e-3 + i;
+  const double x = vin[threadIdx.x & 31], y = vin[(threadIdx.x + 1) & 31];
+  for (int it = 0; it < ITERS; ++it)
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+#pragma unroll
+      for (int i = 0; i < NACC; ++i) a[i] = fma(a[i], x, y);
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < NACC; ++i) s += a[i];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+void run64(int bps) {
+  double *out, *vin; cudaMalloc(&out, 148 * 8 * 256 * 8); cudaMalloc(&vin, 256); cudaMemset(vin, 0, 256);
+  cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int grid = 148 * bps;
+  kern64<<<grid, 256>>>(out, vin); cudaDeviceSynchronize();
+  cudaEventRecord(e0);
+  for (int r = 0; r < 5; ++r) kern64<<<grid, 256>>>(out, vin);
+  cudaEventRecord(e1); cudaEventSynchronize(e1);
+  float ms; cudaEventElapsedTime(&ms, e0, e1); ms /= 5;
+  const double fma = (double)grid * 256 * ITERS * 8.0 * NACC;
+  printf("%-28s blocks/SM=%d: %.3f ms  %.1f FMA/clk/SM (at 1.965 GHz)\n", "DFMA  R,R,R", bps, ms, fma / (ms * 1e-3) / 148 / 1.965e9);
+  cudaFree(out); cudaFree(vin);
+}
 template <int FORM> void run(const char *name, int blocks_per_sm, float *out, float *vin) {
   Coefs cf; for (int i = 0; i < 64; ++i) cf.k[i] = 0.5f + 1e-3f * i;
   cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
@@ -86,6 +116,7 @@ int main() {
     run<6>("FFMA  acc+=R*UR", bps, out, vin);
     run<7>("FFMA2 acc+=R*URbcast", bps, out, vin);
   }
+  run64(1); run64(2);
   runlat<0>("FFMA  R,UR,R", out, vin);
   runlat<1>("FFMA2 R,URpair,R", out, vin);
   runlat<2>("FFMA2 acc+=R*URpair", out, vin);
