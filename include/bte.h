@@ -41,8 +41,8 @@ typedef enum {
   BTE_OK = 0,
   BTE_ERR_INVALID_ARG = 1, /* sizes <= 0, C/v/tau <= 0, non-unit s, unpaired PERIODIC, dim/nz mismatch,
                               no solid cell, interface_bc PERIODIC, NULL where a pointer is required */
-  BTE_ERR_QUADRATURE = 2,  /* |sum w - 4pi| > 1e-6*4pi; a SPECULAR face whose axis reflection does not
-                              map the direction set onto itself (with equal weights) */
+  BTE_ERR_QUADRATURE = 2,  /* |sum w - 4pi| > 1e-6*4pi; with a SPECULAR face: |sum w s| > 1e-9*4pi, or an axis
+                              reflection that does not map the direction set onto itself (equal weights) */
   BTE_ERR_WORKSPACE = 3,   /* workspace NULL, misaligned (256 B) or smaller than bte_workspace_bytes */
   BTE_ERR_CUDA = 4,        /* any CUDA runtime error (bte_last_cuda_error gives the code) */
   BTE_ERR_UNSUPPORTED = 5  /* valid problem outside this build: SPECULAR interface_bc; coefficient table
@@ -52,10 +52,13 @@ typedef enum {
 /* Eq. 5 / Eq. 6 / Eq. 7; PERIODIC: BASELINE.json configs[3] */
 typedef enum { BTE_BC_ISOTHERMAL = 0, BTE_BC_DIFFUSE = 1, BTE_BC_SPECULAR = 2, BTE_BC_PERIODIC = 3 } bte_bc_type;
 
-/* BTE_FP64: everything fp64.  BTE_FP32_STORE_FP64_ACC: cell inputs, tables, recurrence, wavefront
- * buffers and the lagged boundary store in fp32; the moment sum over the <=16 directions of one
- * (octant, band) work item is an fp32 partial, every further sum (bands, octants, cells, residual
- * norms) and the dT division are fp64 (reading G15). */
+/* BTE_FP64: everything fp64.  BTE_FP32_STORE_FP64_ACC (reading G15, as built): cell inputs, tables,
+ * recurrence, wavefront buffers and the lagged boundary store are fp32.  Moments: on the fast path
+ * (bte_kernel_path == 2) the sum over the 16 directions and all bands of ONE OCTANT is fp32 (register partial sums
+ * per band group, added group by group into an fp32 per-octant accumulator, the hemispherical partial sums of
+ * diffuse interfaces likewise); on the generic path only the sum over <= 16 directions of one (octant, band) item is
+ * fp32.  The sums over octants and cells (residual norms), the diffuse-face sums over octants and the dT division
+ * are fp64 on both paths.  Tested against the fp64 oracle at 1e-4 (measured 1e-7 ... 1e-6). */
 typedef enum { BTE_FP64 = 0, BTE_FP32_STORE_FP64_ACC = 1 } bte_precision;
 
 typedef struct { int32_t type; double dT_wall; } bte_bc; /* dT_wall [K] used by ISOTHERMAL only */
@@ -119,8 +122,7 @@ int32_t bte_kernel_launches_per_iteration(const bte_solver *h);
 /* Which sweep kernel serves this problem: 2 = fast path (3-D with even ny and nz, or 2-D with even ny -- run as a
  * slab of two identical layers without z coupling; all-solid or voxel-masked; 16 directions in each octant with
  * mirror-symmetric |s|, w tables; <= 16 bands), 1 = generic path (everything else: 1-D, odd ny / nz, other
- * quadratures).  Both compute the same iteration; the environment variable
- * BTE_FORCE_GENERIC=1 (read by bte_create) forces 1 for testing. */
+ * quadratures).  Both compute the same iteration; bte_set_option(BTE_OPT_FORCE_GENERIC, 1) forces 1 for testing. */
 int32_t bte_kernel_path(const bte_solver *h);
 /* schedule facts for reporting: out[0]=work units per sweep, [1]=CTAs launched, [2]=threads per CTA,
  * [3]=wavefront steps summed over units, [4]=thread-slot updates issued per sweep (occupancy
@@ -134,7 +136,19 @@ void bte_schedule_info(const bte_solver *h, int64_t out[6]);
 bte_status bte_plan_info(const bte_problem *p, int32_t resident_ctas, int64_t out[8]);
 void bte_destroy(bte_solver *h);
 const char *bte_status_string(bte_status s);
+/* Last CUDA runtime error code seen by any entry point of this process (any thread); 0 = none. */
 int32_t bte_last_cuda_error(void);
+
+/* Test / tuning hook: process-wide options consulted by bte_workspace_bytes / bte_create / bte_plan_info (handles
+ * already created are not affected).  The library never reads the environment.  value 0 = default.
+ *   BTE_OPT_FORCE_GENERIC   1: use the generic kernels for every problem
+ *   BTE_OPT_WARPS           2 | 4 | 8: warps per CTA of the fast path (default: by nz)
+ *   BTE_OPT_PUBLISH_PERIOD  2 | 4 | 8 | 16 | 32: steps between progress publications of a warp (default 8; 4 if nx <= 96)
+ *   BTE_OPT_START_SLACK     1..256: extra steps a unit lets the units it follows get ahead before it starts
+ * Returns BTE_ERR_INVALID_ARG for an unknown option. */
+typedef enum { BTE_OPT_FORCE_GENERIC = 0, BTE_OPT_WARPS = 1, BTE_OPT_PUBLISH_PERIOD = 2, BTE_OPT_START_SLACK = 3,
+               BTE_OPT_COUNT_ = 4 } bte_option;
+bte_status bte_set_option(int32_t option, int32_t value);
 
 #ifdef __cplusplus
 }

@@ -33,7 +33,7 @@ EXPORTS = ["bte_workspace_bytes", "bte_create", "bte_iterate", "bte_get_temperat
            "bte_set_temperature", "bte_residual", "bte_solve_host", "bte_set_sweep_timing",
            "bte_get_sweep_timing", "bte_updates_per_sweep",
            "bte_iterations_done", "bte_kernel_launches_per_iteration", "bte_kernel_path", "bte_plan_info", "bte_schedule_info", "bte_destroy",
-           "bte_status_string", "bte_last_cuda_error"]
+           "bte_status_string", "bte_last_cuda_error", "bte_set_option"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -109,8 +109,19 @@ def lib():
         L.bte_status_string.argtypes = [C.c_int]
         L.bte_status_string.restype = C.c_char_p
         L.bte_last_cuda_error.restype = i32
+        L.bte_set_option.argtypes = [i32, i32]
         _lib = L
     return _lib
+
+
+OPTIONS = {"force_generic": 0, "warps": 1, "publish_period": 2, "start_slack": 3}
+
+
+def bte_set_option(name, value) -> None:
+    """Process-wide test / tuning option (include/bte.h bte_set_option); 0 restores the default."""
+    rc = lib().bte_set_option(OPTIONS[name], int(value))
+    if rc:
+        raise BteError(rc, "bte_set_option")
 
 
 def _marshal(p, precision=None):

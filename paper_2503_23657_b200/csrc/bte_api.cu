@@ -16,11 +16,14 @@
 
 #include "bte_kernels.cuh"
 
-static thread_local int g_last_cuda = 0;
+#include <atomic>
+static std::atomic<int> g_last_cuda{0};   // process-wide: bte_last_cuda_error() may be called from any thread
+// Process-wide test / tuning options (bte_set_option): the product never reads the environment.
+static std::atomic<int> g_opt[BTE_OPT_COUNT_];
 #define CK(call)                                                       \
   do {                                                                 \
     cudaError_t e_ = (call);                                           \
-    if (e_ != cudaSuccess) { g_last_cuda = (int)e_; return BTE_ERR_CUDA; } \
+    if (e_ != cudaSuccess) { g_last_cuda.store((int)e_); return BTE_ERR_CUDA; } \
   } while (0)
 
 namespace {
@@ -182,6 +185,15 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
       for (int a = 0; a < 3; ++a) if (key(x, a) != key(y, a)) return key(x, a) < key(y, a);
       return x < y;
     });
+  {   // a SPECULAR face needs a first moment that vanishes (Eq. 7 conserves energy only then): |sum w s| <= 1e-9 * 4 pi
+    bool any_spec = false;
+    for (int f = 0; f < 2 * p->dim; ++f) any_spec = any_spec || p->face_bc[f].type == BTE_BC_SPECULAR;
+    if (any_spec) {
+      double m1[3] = {0, 0, 0};
+      for (int d = 0; d < D; ++d) for (int c = 0; c < 3; ++c) m1[c] += p->w[d] * p->s[3 * d + c];
+      if (std::sqrt(m1[0] * m1[0] + m1[1] * m1[1] + m1[2] * m1[2]) > 1e-9 * kFourPi) return BTE_ERR_QUADRATURE;
+    }
+  }
   for (int a = 0; a < p->dim; ++a) {
     if (p->face_bc[2 * a].type != BTE_BC_SPECULAR && p->face_bc[2 * a + 1].type != BTE_BC_SPECULAR) continue;
     for (int o = 0; o < 8; ++o) {
@@ -289,7 +301,7 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
   // (mirror-symmetric quadrature), <= 16 bands.  Anything else runs the generic kernels above.
   bool v2 = p->dim == 3 && B <= BTE2_MAXB && p->nx <= 60000 && p->ny % 2 == 0 && p->nz % 2 == 0;
   pl.masked2 = nsolid != N;
-  if (const char *e = std::getenv("BTE_FORCE_GENERIC")) if (e[0] == '1') v2 = false;
+  if (g_opt[BTE_OPT_FORCE_GENERIC].load() == 1) v2 = false;
   for (int o = 0; o < 8 && v2; ++o) {
     if ((int)od[o].size() != BTE2_P) v2 = false;
     for (int b = 0; b < B && v2; ++b) {   // same table up to rounding of the mirrored direction cosines
@@ -302,19 +314,17 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
   if (v2) {
     Bte2Dev &d = pl.d2;
     int W = p->nz >= 48 ? 8 : (p->nz <= 4 ? 2 : 4);   // 2 warps: thin slabs (the two-layer form of 2-D problems)
-    if (const char *e = std::getenv("BTE_V2_W")) { const int w = std::atoi(e); if (w == 2 || w == 4 || w == 8) W = w; }
+    { const int w = g_opt[BTE_OPT_WARPS].load(); if (w == 2 || w == 4 || w == 8) W = w; }
     d.nx = p->nx; d.ny = p->ny; d.nz = p->nz; d.B = B; d.W = W;
     d.nty = (p->ny + 63) / 64; d.ntz = (p->nz + 2 * W - 1) / (2 * W); d.NU = p->nx + 31;
-    d.nsteps = p->nx + 31 + W - 1;
-#ifdef BTE2_ENABLE_DBG
-    if (const char *e = std::getenv("BTE_V2_DBG")) d.dbg = std::atoi(e);   // timing experiments (skips parts of the kernel)
-#endif
-    d.pub_mask = (p->nx <= 96 ? BTE2_PUB / 2 : BTE2_PUB) - 1; d.slack = BTE2_SLACK;   // short rows: publish progress twice as often (measured)
-    if (const char *e = std::getenv("BTE_V2_PUB")) { const int v = std::atoi(e); if (v == 4 || v == 8 || v == 16 || v == 32) d.pub_mask = v - 1; }
-    if (const char *e = std::getenv("BTE_V2_SLACK")) { const int v = std::atoi(e); if (v >= 0 && v <= 256) d.slack = v; }
+    d.nsteps = p->nx + 32 + W - 1;                   // nx + 32 local steps per warp, warp K one step behind warp K-1
+    d.pub_mask = (p->nx <= 96 ? BTE2_PUB / 2 : BTE2_PUB) - 1; d.slack = 0;   // short rows: publish progress twice as often (measured)
+    { const int v = g_opt[BTE_OPT_PUBLISH_PERIOD].load(); if (v == 2 || v == 4 || v == 8 || v == 16 || v == 32) d.pub_mask = v - 1; }
+    { const int v = g_opt[BTE_OPT_START_SLACK].load(); if (v > 0 && v <= 256) d.slack = v; }
     d.NS = (int64_t)p->nz * d.nty * d.NU * 64;
     d.ncell = N; d.src_mod = N; d.inv_sumCtau = dv.inv_sumCtau;
     const int NBmax = dv.fp32 ? 2 : 1, G = (B + NBmax - 1) / NBmax;
+    d.G = G;
     for (int b = 0; b < B; ++b) {
       const double *blk = pl.coef.data() + pl.item_coef[b];
       for (int q = 0; q < BTE2_P; ++q) {
@@ -363,8 +373,8 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
     d.n_units = (int32_t)pl.units2.size();
     const size_t nch = BTE2_P * tsz / 16;
     pl.x2_chunks = (size_t)d.ntz * d.nty * B * W * 2 * 2 * nch * 32;
-    pl.y2_slot = (size_t)d.ntz * B * W * d.nx * 2 * nch;
-    pl.z2_slot = (size_t)d.nty * B * d.NU * 2 * nch * 32;
+    pl.y2_slot = (size_t)d.ntz * G * W * d.nx * NBmax * 2 * nch;      // rows of whole band groups (bte_sweep2.cuh layouts)
+    pl.z2_slot = (size_t)d.nty * G * d.NU * NBmax * 2 * nch * 32;
     pl.y2_chunks = (size_t)(d.nty + 2) * pl.y2_slot;
     pl.z2_chunks = (size_t)(d.ntz + 2) * pl.z2_slot;
     int64_t off = 0;
@@ -387,7 +397,7 @@ bte_status build_plan(const bte_problem *p, Plan &pl) {
   bte_status st = build_plan_impl(p, pl);
   pl.user_ncell = pl.dev.ncell; pl.user_nsolid = pl.dev.nsolid;
   if (st != BTE_OK || pl.v2 || p->dim != 2 || p->ny % 2 != 0) return st;
-  if (const char *e = std::getenv("BTE_FORCE_GENERIC")) if (e[0] == '1') return st;
+  if (g_opt[BTE_OPT_FORCE_GENERIC].load() == 1) return st;
   const size_t N = (size_t)p->nx * p->ny;
   std::vector<uint8_t> mask2;
   std::vector<double> Q2;
@@ -437,7 +447,7 @@ size_t bind(Plan &pl, unsigned char *ws) {
     pl.state_begin = off;
     d.Gi = d.n_iface ? take((size_t)d.n_iface * d.B * tsz) : nullptr;
     d.Hd = (d.n_iface && d.iface_type == 1) ? take((size_t)6 * N * d.B * 4 * tsz) : nullptr;
-    d.prog = (int32_t *)take((size_t)d.n_units * 4);
+    d.prog = (int32_t *)take((size_t)d.n_units * d.W * 4);
     d.ticket = (int32_t *)take(256);
     dv.red = (double *)take((size_t)(4 * dv.n_red_blocks + 4) * 8);
     dv.dT = (double *)take(N * 8);
@@ -500,10 +510,12 @@ void order_units2(Plan &pl, int slots) {
   }
   auto allowed = [&](int u) {
     const int deps[3] = {U[u].dep_y, U[u].dep_z, U[u].dep_prev};
-    const int lag[3] = {33, W + 1, 1};
+    // steps the followed unit must be ahead: y outflow lag + prefetch distance; z: its last warp trails its first by W - 1
+    const int D = pl.dev.fp32 ? BTE2_DIST(W, float) : BTE2_DIST(W, double);
+    const int lag[3] = {BTE2_YLAG + D, W + D, 1};
     double a = 0;
     for (int k = 0; k < 3; ++k)
-      if (deps[k] >= 0) a = std::max(a, start[deps[k]] + (lag[k] + (pl.dev.fp32 ? BTE2_DIST(W, float) : BTE2_DIST(W, double)) + pl.d2.slack + pl.d2.pub_mask + 1) * steptime[deps[k]]);
+      if (deps[k] >= 0) a = std::max(a, start[deps[k]] + (lag[k] + pl.d2.slack + pl.d2.pub_mask + 2) * steptime[deps[k]]);
     return a;
   };
   typedef std::pair<double, int> Key;
@@ -590,7 +602,7 @@ bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t
   const int bgrid = h->num_sms * 8;
   for (int it = 0; it < n; ++it) {
     const int ep = (int)(h->iters % 30000) + 1;
-    if (ep == 1 && h->iters > 0) CK(cudaMemsetAsync(d.prog, 0, (size_t)d.n_units * 4, st));
+    if (ep == 1 && h->iters > 0) CK(cudaMemsetAsync(d.prog, 0, (size_t)d.n_units * d.W * 4, st));
     d.epoch = ep;
     d.fill_iso = h->iters == 0;
     {   // ghost planes to fill: diffuse faces every iteration, isothermal faces once (specular / periodic: none)
@@ -643,7 +655,7 @@ bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t
 template <typename T, int W>
 bte_status setup_sweep2_W(bte_solver *h) {
   Plan &pl = h->pl;
-  pl.smem2 = sizeof(Bte2Smem<T, sizeof(T) == 4 ? 2 : 1, W, BTE2_DIST(W, T)>);
+  pl.smem2 = sizeof(Bte2Smem<T, BTE2_NBMAX(T), W, BTE2_DIST(W, T)>);
   int occ = 0;
   if (pl.masked2) {
     CK(cudaFuncSetAttribute(bte2_sweep_kernel<T, W, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem2));
@@ -652,7 +664,7 @@ bte_status setup_sweep2_W(bte_solver *h) {
     CK(cudaFuncSetAttribute(bte2_sweep_kernel<T, W, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem2));
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bte2_sweep_kernel<T, W, false>, W * 32, pl.smem2));
   }
-  if (occ < 1) { g_last_cuda = (int)cudaErrorLaunchOutOfResources; return BTE_ERR_CUDA; }
+  if (occ < 1) { g_last_cuda.store((int)cudaErrorLaunchOutOfResources); return BTE_ERR_CUDA; }
   h->sweep_grid = (int)std::min<int64_t>(pl.d2.n_units, (int64_t)h->num_sms * occ);
   pl.nthreads = W * 32;
   return BTE_OK;
@@ -690,7 +702,7 @@ bte_status setup_sweep(bte_solver *h) {
   CK(cudaFuncSetAttribute(bte_sweep_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
   int occ = 0;
   CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bte_sweep_kernel<T>, pl.nthreads, pl.smem));
-  if (occ < 1) { g_last_cuda = (int)cudaErrorLaunchOutOfResources; return BTE_ERR_CUDA; }
+  if (occ < 1) { g_last_cuda.store((int)cudaErrorLaunchOutOfResources); return BTE_ERR_CUDA; }
   h->sweep_grid = (int)std::min<int64_t>(pl.dev.n_units, (int64_t)h->num_sms * occ);
   return BTE_OK;
 }
@@ -720,7 +732,7 @@ bte_status bte_create(const bte_problem *p, void *d_workspace, size_t bytes, voi
   Plan &pl = h->pl;
   BteDev &dv = pl.dev;
   auto fail = [&](bte_status e) { delete h; return e; };
-#define CKD(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { g_last_cuda = (int)e_; return fail(BTE_ERR_CUDA); } } while (0)
+#define CKD(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { g_last_cuda.store((int)e_); return fail(BTE_ERR_CUDA); } } while (0)
   int devid = 0;
   CKD(cudaGetDevice(&devid));
   CKD(cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, devid));
@@ -949,6 +961,12 @@ const char *bte_status_string(bte_status s) {
   }
   return "unknown";
 }
-int32_t bte_last_cuda_error(void) { return g_last_cuda; }
+int32_t bte_last_cuda_error(void) { return g_last_cuda.load(); }
+
+bte_status bte_set_option(int32_t option, int32_t value) {
+  if (option < 0 || option >= BTE_OPT_COUNT_) return BTE_ERR_INVALID_ARG;
+  g_opt[option].store(value);
+  return BTE_OK;
+}
 
 }  // extern "C"

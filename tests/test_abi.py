@@ -82,3 +82,42 @@ def test_product_does_not_import_the_oracle():
         if f.endswith((".py", ".cpp", ".h")):
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert "paper_2503_23657_b200" not in txt.replace("paper_2503_23657_b200/csrc", "") or f == "bte_ref.h"
+
+
+def test_options_replace_environment_variables(L):
+    """bte_set_option is the only test / tuning hook: the product never reads the environment."""
+    for root, _, files in os.walk(os.path.join(ROOT, "paper_2503_23657_b200")):
+        for f in files:
+            if f.endswith((".cu", ".cuh", ".h")):
+                assert "getenv" not in open(os.path.join(root, f)).read(), f
+    p = W.config(4, grid=(40, 34, 20))
+    assert bte.bte_plan_info(p)["kernel_path"] == 2
+    try:
+        bte.bte_set_option("force_generic", 1)
+        assert bte.bte_plan_info(p)["kernel_path"] == 1
+        bte.bte_set_option("force_generic", 0)
+        bte.bte_set_option("warps", 4)
+        assert bte.bte_plan_info(p)["warps_per_cta"] == 4
+    finally:
+        bte.bte_set_option("force_generic", 0)
+        bte.bte_set_option("warps", 0)
+    assert bte.bte_plan_info(p)["kernel_path"] == 2
+    assert L.bte_set_option(99, 1) == 1 and L.bte_set_option(-1, 1) == 1     # BTE_ERR_INVALID_ARG
+
+
+def test_specular_face_needs_a_vanishing_first_moment(L):
+    """|sum w s| > 1e-9 * 4 pi with a SPECULAR face -> BTE_ERR_QUADRATURE (Eq. 7 conserves energy only
+    for a table whose first moment vanishes).  The skewed table below keeps sum w = 4 pi and stays closed under the
+    x and y mirror flips (weights equal within each mirror orbit) but has a net z moment."""
+    p = W.config(4, grid=(8, 8, 8))                     # x, y faces specular
+    w = p.w.copy()
+    up = p.s[:, 2] > 0
+    w[up] *= 1.0 + 1e-6
+    w *= 4 * np.pi / w.sum()
+    bad = W.config(4, grid=(8, 8, 8)); bad.w = w
+    pr, keep = bte._marshal(bad)
+    out = (C.c_int64 * 8)()
+    assert L.bte_plan_info(C.byref(pr), 148, out) == 2  # BTE_ERR_QUADRATURE
+    ok = W.config(2, grid=(8, 8, 8)); ok.w = w          # no specular face: the same table is accepted
+    pr, keep = bte._marshal(ok)
+    assert L.bte_plan_info(C.byref(pr), 148, out) == 0

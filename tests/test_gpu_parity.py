@@ -27,6 +27,19 @@ def bte():
     return m
 
 
+@pytest.fixture
+def option(bte):
+    """bte_set_option for the duration of one test (the library never reads the environment)."""
+    used = []
+
+    def set_(name, value):
+        bte.bte_set_option(name, value)
+        used.append(name)
+    yield set_
+    for name in used:
+        bte.bte_set_option(name, 0)
+
+
 def errors(dT, q, dT_ref, q_ref):
     eT = np.max(np.abs(dT - dT_ref)) / max(np.max(np.abs(dT_ref)), 1e-300)
     dq = np.sqrt(((q - q_ref) ** 2).sum(axis=0))
@@ -90,20 +103,20 @@ def test_shrunken_configs(bte, k, prec):
 
 @pytest.mark.parametrize("k", [2, 4])
 @pytest.mark.parametrize("prec", [W.FP64, W.FP32_STORE_FP64_ACC])
-def test_shrunken_configs_fast_path(bte, k, prec, monkeypatch):
+def test_shrunken_configs_fast_path(bte, k, prec, option):
     """The 3-D unmasked configs on the fast sweep kernel, and the same problem forced onto the generic one."""
     p = W.config(k, grid=SHRUNK_FAST[k])
     assert bte.Solver(p, precision=prec).kernel_path == 2
     check(bte, p, 30, precision=prec, checkpoints=(1, 2, 10))
-    monkeypatch.setenv("BTE_FORCE_GENERIC", "1")
+    option("force_generic", 1)
     assert bte.Solver(p, precision=prec).kernel_path == 1
     check(bte, p, 6, precision=prec, checkpoints=(1,))
 
 
-@pytest.mark.parametrize("warps", ["4", "8"])
-def test_fast_path_tile_heights(bte, warps, monkeypatch):
+@pytest.mark.parametrize("warps", [4, 8])
+def test_fast_path_tile_heights(bte, warps, option):
     """Both CTA shapes of the fast path (tiles of 8 and 16 rows in z), several z tiles, periodic + specular faces."""
-    monkeypatch.setenv("BTE_V2_W", warps)
+    option("warps", warps)
     p = W.config(4, grid=(37, 66, 52))
     p.face_bc = [(W.BC_PERIODIC, 0.0), (W.BC_PERIODIC, 0.0), (W.BC_SPECULAR, 0.0), (W.BC_DIFFUSE, 0.0),
                  (W.BC_ISOTHERMAL, 0.1), (W.BC_SPECULAR, 0.0)]
@@ -124,13 +137,13 @@ def test_masked_grids_on_the_fast_path(bte, seed):
     check(bte, p, 12, precision=W.FP32_STORE_FP64_ACC)
 
 
-def test_finfet_mask_fast_vs_generic(bte, monkeypatch):
+def test_finfet_mask_fast_vs_generic(bte, option):
     """Config 3 (fin + slab, diffuse interfaces, periodic x) at a size with several z tiles on both kernel paths."""
     p = W.config(3, grid=(36, 68, 40))
     assert bte.Solver(p).kernel_path == 2
     check(bte, p, 20, checkpoints=(1, 5))
     check(bte, p, 6, precision=W.FP64, checkpoints=(1,))
-    monkeypatch.setenv("BTE_FORCE_GENERIC", "1")
+    option("force_generic", 1)
     assert bte.Solver(p).kernel_path == 1
     check(bte, p, 6, precision=W.FP64, checkpoints=(1,))
 
@@ -304,13 +317,13 @@ def test_progress_epoch_wraps_without_hanging(bte):
     assert np.abs(b.cpu().numpy() - ref.temperature()).max() <= 1e-8 * np.abs(ref.temperature()).max()
 
 
-@pytest.mark.parametrize("warps", ["4", "8"])
+@pytest.mark.parametrize("warps", [4, 8])
 @pytest.mark.parametrize("prec", [W.FP64, W.FP32_STORE_FP64_ACC])
 @pytest.mark.parametrize("k", [3, 4])
-def test_repeated_runs_are_bitwise_identical(bte, k, prec, warps, monkeypatch):
+def test_repeated_runs_are_bitwise_identical(bte, k, prec, warps, option):
     """Race detector for the tile pipeline (inter-tile progress flags, staged faces, accumulator hand-over between band
     groups): several y and z tiles, every run of the same problem must give the same bits."""
-    monkeypatch.setenv("BTE_V2_W", warps)
+    option("warps", warps)
     p = W.config(k, grid=(45, 130, 36) if k == 4 else (40, 68, 40))
     ref = None
     for _ in range(5):
