@@ -54,6 +54,7 @@ struct Plan {
   std::vector<uint32_t> codeP[4];
   Bte2Dev d2{};
   std::vector<Bte2Unit> units2;
+  std::vector<int32_t> gorder2;          // unit ids in ticket order, band group after band group
   Bte2Coefs<float> cf32{};
   Bte2Coefs<double> cf64{};
   size_t smem2 = 0;
@@ -434,6 +435,7 @@ size_t bind(Plan &pl, unsigned char *ws) {
     Bte2Dev &d = pl.d2;
     const size_t NS2 = (size_t)d.NS;
     d.units = (const Bte2Unit *)take(pl.units2.size() * sizeof(Bte2Unit));
+    d.gorder = (const int32_t *)take(pl.units2.size() * 4);
     if (pl.masked2) {
       d.code = dv.code;
       for (int c = 0; c < 4; ++c) d.codeP[c] = (const uint32_t *)take((size_t)(dv.nz / 2) * d.nty * d.NU * 32 * 4);
@@ -493,56 +495,80 @@ size_t bind(Plan &pl, unsigned char *ws) {
   return off;
 }
 
-// Ticket order of the fast path = start order of a list schedule simulated on `slots` resident CTAs:
-// a unit may start once every unit it follows is lag + BTE2_SLACK steps ahead, so that the per-step
-// dependency polls of the kernel (which stay in place for correctness) almost never have to wait.
+// Schedule of the fast path.  Every CTA serves one band group (bte_sweep2.cuh): the `slots` resident CTAs are shared out
+// to the groups in proportion to their work (a group of one band costs half a group of two), and each group's ticket
+// order is the start order of a list schedule simulated with these per-group CTA pools: a unit may start once every
+// unit it follows is `lag` steps ahead, so that the per-step dependency polls of the kernel (which stay in place for
+// correctness) almost never have to wait, and the G groups work on the same tile at the same time (L2 reuse of the
+// cell inputs and of the accumulator rows).  Deadlock-free for any slots >= G: group g only follows group g - 1 and
+// earlier units of its own list.
 void order_units2(Plan &pl, int slots) {
   std::vector<Bte2Unit> &U = pl.units2;
-  const int n = (int)U.size(), W = pl.d2.W, nsteps = pl.d2.nsteps;
+  Bte2Dev &d = pl.d2;
+  const int n = (int)U.size(), W = d.W, nsteps = d.nsteps, G = d.G;
   const int NBmax = pl.dev.fp32 ? 2 : 1;
+  // CTAs per group
+  std::vector<int> ng(G, 0), cnt(G, 1);
+  std::vector<double> wg(G, 1.0);
+  for (int u = 0; u < n; ++u) { ++ng[U[u].g]; wg[U[u].g] = (double)U[u].nb / NBmax; }
+  slots = std::max(slots, G);
+  double wsum = 0;
+  for (int g = 0; g < G; ++g) wsum += wg[g];
+  int used = 0;
+  for (int g = 0; g < G; ++g) { cnt[g] = std::max(1, std::min(ng[g], (int)std::floor(slots * wg[g] / wsum))); used += cnt[g]; }
+  for (;;) {   // hand the remaining CTAs to the group with the longest queue per CTA
+    int best = -1; double load = 0;
+    for (int g = 0; g < G; ++g) if (cnt[g] < ng[g] && ng[g] * wg[g] / cnt[g] > load) { load = ng[g] * wg[g] / cnt[g]; best = g; }
+    if (best < 0 || used >= slots) break;
+    ++cnt[best]; ++used;
+  }
+  for (int g = 0; g < BTE2_MAXB; ++g) d.cta_count[g] = g < G ? cnt[g] : 0;
+  // list schedule
   std::vector<double> start(n, -1.0), steptime(n);
-  std::vector<int> ndep(n, 0), order;
+  std::vector<int> ndep(n, 0);
   std::vector<std::vector<int>> succ(n);
   for (int u = 0; u < n; ++u) {
     steptime[u] = (double)U[u].nb / NBmax;
     const int deps[3] = {U[u].dep_y, U[u].dep_z, U[u].dep_prev};
-    for (int d : deps) if (d >= 0) { ++ndep[u]; succ[d].push_back(u); }
+    for (int dd : deps) if (dd >= 0) { ++ndep[u]; succ[dd].push_back(u); }
   }
+  const int D = pl.dev.fp32 ? BTE2_DIST(W, float) : BTE2_DIST(W, double);
   auto allowed = [&](int u) {
     const int deps[3] = {U[u].dep_y, U[u].dep_z, U[u].dep_prev};
     // steps the followed unit must be ahead: y outflow lag + prefetch distance; z: its last warp trails its first by W - 1
-    const int D = pl.dev.fp32 ? BTE2_DIST(W, float) : BTE2_DIST(W, double);
     const int lag[3] = {BTE2_YLAG + D, W + D, 1};
     double a = 0;
     for (int k = 0; k < 3; ++k)
-      if (deps[k] >= 0) a = std::max(a, start[deps[k]] + (lag[k] + pl.d2.slack + pl.d2.pub_mask + 2) * steptime[deps[k]]);
+      if (deps[k] >= 0) a = std::max(a, start[deps[k]] + (lag[k] + d.slack + d.pub_mask + 2) * steptime[deps[k]]);
     return a;
   };
   typedef std::pair<double, int> Key;
-  std::priority_queue<Key, std::vector<Key>, std::greater<Key>> ready, freeslot;
-  for (int u = 0; u < n; ++u) if (ndep[u] == 0) ready.push({0.0, u});
-  for (int k = 0; k < std::max(slots, 1); ++k) freeslot.push({0.0, k});
-  order.reserve(n);
-  while (!ready.empty()) {
-    const Key f = freeslot.top(); freeslot.pop();
-    const Key r = ready.top(); ready.pop();
-    const int u = r.second;
-    start[u] = std::max(f.first, r.first);
-    freeslot.push({start[u] + nsteps * steptime[u], f.second});
-    order.push_back(u);
-    for (int v : succ[u]) if (--ndep[v] == 0) ready.push({allowed(v), v});
+  typedef std::priority_queue<Key, std::vector<Key>, std::greater<Key>> Heap;
+  std::vector<Heap> ready(G), freeslot(G);
+  for (int g = 0; g < G; ++g) for (int k = 0; k < cnt[g]; ++k) freeslot[g].push({0.0, k});
+  for (int u = 0; u < n; ++u) if (ndep[u] == 0) ready[U[u].g].push({0.0, u});
+  std::vector<std::vector<int>> order(G);
+  for (int done = 0; done < n; ++done) {
+    int bg = -1; double bt = 0;
+    for (int g = 0; g < G; ++g) {
+      if (ready[g].empty()) continue;
+      const double t = std::max(ready[g].top().first, freeslot[g].top().first);
+      if (bg < 0 || t < bt) { bg = g; bt = t; }
+    }
+    if (bg < 0) break;                    // cannot happen: the dependency graph is acyclic
+    const int u = ready[bg].top().second; ready[bg].pop();
+    const Key f = freeslot[bg].top(); freeslot[bg].pop();
+    start[u] = bt;
+    freeslot[bg].push({bt + nsteps * steptime[u], f.second});
+    order[bg].push_back(u);
+    for (int v : succ[u]) if (--ndep[v] == 0) ready[U[v].g].push({allowed(v), v});
   }
-  std::vector<int> newid(n);
-  for (int k = 0; k < n; ++k) newid[order[k]] = k;
-  std::vector<Bte2Unit> out(n);
-  for (int k = 0; k < n; ++k) {
-    Bte2Unit x = U[order[k]];
-    if (x.dep_y >= 0) x.dep_y = newid[x.dep_y];
-    if (x.dep_z >= 0) x.dep_z = newid[x.dep_z];
-    if (x.dep_prev >= 0) x.dep_prev = newid[x.dep_prev];
-    out[k] = x;
+  pl.gorder2.clear();
+  for (int g = 0; g < G; ++g) {
+    d.gfirst[g] = (int32_t)pl.gorder2.size();
+    pl.gorder2.insert(pl.gorder2.end(), order[g].begin(), order[g].end());
   }
-  U.swap(out);
+  for (int g = G; g <= BTE2_MAXB; ++g) d.gfirst[g] = (int32_t)pl.gorder2.size();
 }
 
 }  // namespace
@@ -591,8 +617,11 @@ bte_status skew(bte_solver *h, const double *src, double scale, int which, cudaS
 
 template <typename T, int W>
 void launch_sweep2(bte_solver *h, const Bte2Coefs<T> &cf, cudaStream_t st) {
-  if (h->pl.masked2) bte2_sweep_kernel<T, W, true><<<h->sweep_grid, W * 32, h->pl.smem2, st>>>(h->pl.d2, cf);
-  else bte2_sweep_kernel<T, W, false><<<h->sweep_grid, W * 32, h->pl.smem2, st>>>(h->pl.d2, cf);
+  int cmax = 1;
+  for (int g = 0; g < h->pl.d2.G; ++g) cmax = std::max(cmax, h->pl.d2.cta_count[g]);
+  const dim3 grid((unsigned)cmax, (unsigned)h->pl.d2.G);   // CTA (x, y): band group y; it leaves at once if x >= cta_count[y]
+  if (h->pl.masked2) bte2_sweep_kernel<T, W, true><<<grid, W * 32, h->pl.smem2, st>>>(h->pl.d2, cf);
+  else bte2_sweep_kernel<T, W, false><<<grid, W * 32, h->pl.smem2, st>>>(h->pl.d2, cf);
 }
 
 template <typename T>
@@ -665,7 +694,7 @@ bte_status setup_sweep2_W(bte_solver *h) {
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bte2_sweep_kernel<T, W, false>, W * 32, pl.smem2));
   }
   if (occ < 1) { g_last_cuda.store((int)cudaErrorLaunchOutOfResources); return BTE_ERR_CUDA; }
-  h->sweep_grid = (int)std::min<int64_t>(pl.d2.n_units, (int64_t)h->num_sms * occ);
+  h->sweep_grid = std::max(pl.d2.G, h->num_sms * occ);   // resident CTA budget (order_units2 shares it out to the band groups)
   pl.nthreads = W * 32;
   return BTE_OK;
 }
@@ -745,6 +774,9 @@ bte_status bte_create(const bte_problem *p, void *d_workspace, size_t bytes, voi
   if (pl.v2) {
     order_units2(pl, h->sweep_grid);
     CKD(cudaMemcpyAsync((void *)pl.d2.units, pl.units2.data(), pl.units2.size() * sizeof(Bte2Unit), cudaMemcpyHostToDevice, s));
+    CKD(cudaMemcpyAsync((void *)pl.d2.gorder, pl.gorder2.data(), pl.gorder2.size() * 4, cudaMemcpyHostToDevice, s));
+    h->sweep_grid = 0;
+    for (int g = 0; g < pl.d2.G; ++g) h->sweep_grid += pl.d2.cta_count[g];   // CTAs that take tickets
     if (pl.masked2) {
       for (int c = 0; c < 4; ++c)
         CKD(cudaMemcpyAsync((void *)pl.d2.codeP[c], pl.codeP[c].data(), pl.codeP[c].size() * 4, cudaMemcpyHostToDevice, s));
@@ -908,6 +940,22 @@ bte_status bte_plan_info(const bte_problem *p, int32_t resident_ctas, int64_t ou
   }
   order_units2(pl, std::max(resident_ctas, 1));
   bool topo = true, same = true;
+  {   // every group's ticket list holds exactly its units, each after the units of the same group it follows
+    std::vector<int> pos(pl.units2.size(), -1);
+    for (size_t k = 0; k < pl.gorder2.size(); ++k) pos[pl.gorder2[k]] = (int)k;
+    int ctas = 0;
+    for (int g = 0; g < pl.d2.G; ++g) {
+      ctas += pl.d2.cta_count[g];
+      topo = topo && pl.d2.cta_count[g] >= 1;
+      for (int k = pl.d2.gfirst[g]; k < pl.d2.gfirst[g + 1]; ++k) topo = topo && pl.units2[pl.gorder2[k]].g == g;
+    }
+    topo = topo && pl.gorder2.size() == pl.units2.size() && ctas <= std::max(resident_ctas, pl.d2.G);
+    for (size_t u = 0; u < pl.units2.size(); ++u) {
+      const Bte2Unit &U = pl.units2[u];
+      topo = topo && pos[u] >= 0;
+      for (int d : {U.dep_y, U.dep_z}) if (d >= 0) topo = topo && pos[d] < pos[u];
+    }
+  }
   for (size_t u = 0; u < pl.units2.size(); ++u) {
     const Bte2Unit &U = pl.units2[u];
     for (int d : {U.dep_y, U.dep_z, U.dep_prev}) topo = topo && d < (int)u;

@@ -25,10 +25,16 @@
 // K+1 to have released the buffer it overwrites (mbarrier zempty); the warps of a CTA drift against
 // each other, so one warp's memory-side work overlaps the other warps' arithmetic.
 //
-// Scheduling.  Persistent CTAs take tickets in a topological unit order.  Dependencies between
-// tiles are tracked per WARP and per STEP, not per tile: every warp publishes its step count
-// (release store) every BTE2_PUB steps, and the downstream tile in y / z (and the next band group on
-// the same tile, whose additions to the accumulator must come after this one's) stays behind it.
+// Scheduling.  Every persistent CTA serves ONE band group for the whole launch (the group is blockIdx.y) and takes tickets from that group's unit list, which is in topological order.
+// So the band index is a function of blockIdx alone: the compiler keeps the coefficient addressing on
+// the uniform datapath (measured on the SASS: values that come from memory, from warp votes or even
+// from kernel parameters do not qualify inside this kernel, and the FFMA2s then take three vector
+// operands and a constant load each), and the CTAs of the G groups sweep the same tile at the same time,
+// each a few steps behind the previous group, so the cell inputs and the accumulator rows of a tile
+// stay in the L2 between the groups.  Dependencies between tiles are tracked per WARP and per STEP,
+// not per tile: every warp publishes its step count (release store) every BTE2_PUB steps, and the
+// downstream tile in y / z (and the next band group on the same tile, whose additions to the
+// accumulator must come after this one's) stays behind it.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -78,8 +84,11 @@ struct Bte2Dev {
   void *dTQ[4];                     // T2 [NS]: (dT, Q / sum C) per x/y-flip class
   Bte2Oct oct[8];
   const Bte2Unit *units;
+  const int32_t *gorder;            // unit ids in ticket order, group after group: group g owns [gfirst[g], gfirst[g+1])
+  int32_t gfirst[BTE2_MAXB + 1];
+  int32_t cta_count[BTE2_MAXB];     // grid = (max cta_count, G): CTA (x, y) serves band group y; it leaves at once if x >= cta_count[y]
   int32_t *prog;                    // [n_units][W] epoch << 16 | steps published by warp K of the unit
-  int32_t *ticket;
+  int32_t *ticket;                  // [BTE2_MAXB] one ticket counter per band group
   // boundary conditions (box faces x-,x+,y-,y+,z-,z+) and the update kernel
   int32_t face_type[6];
   double face_e0[6][BTE2_MAXB];     // isothermal inflow C_b dT_w / 4pi (Eq. 5)
@@ -158,33 +167,17 @@ __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)_
 __device__ __forceinline__ void mbar_init(uint64_t *b, int count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
 }
-__device__ __forceinline__ void mbar_inval(uint64_t *b) { asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(b)) : "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void mbar_arrive(uint64_t *b) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory"); }
 __device__ __forceinline__ void mbar_expect(uint64_t *b, unsigned bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ bool mbar_try(uint64_t *b, unsigned parity) {
-  unsigned ok;
-  asm volatile("{\n.reg .pred P1;\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\nselp.u32 %0, 1, 0, P1;\n}" : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
-  return ok != 0;
-}
-#ifdef BTE2_WATCHDOG   // debug builds: a wait that spins too long reports where it is; much later every stuck wait gives up
-__device__ int g_bte2_abort;
-#define BTE2_WD_DECL long long wd_n = 0
-#define BTE2_WD_POLL(kind, a, b, c, d)                                                                             \
-  if (++wd_n == (kind[0] == 'd' ? (1ll << 21) : (1ll << 13))) {                                                    \
-    if ((threadIdx.x & 31) == 0 || kind[0] == 'd') printf("WD cta %d warp %d lane %d kind %s: %d %d %d %d\n", blockIdx.x, threadIdx.x >> 5, threadIdx.x & 31, kind, a, b, c, d); \
-  }                                                                                                                \
-  if (wd_n == (kind[0] == 'd' ? (1ll << 23) : (1ll << 15))) atomicExch(&g_bte2_abort, 1);                          \
-  if ((wd_n & 0xfff) == 0 && wd_n > (kind[0] == 'd' ? (1ll << 21) : (1ll << 13)) && *(volatile int *)&g_bte2_abort) break;
-#else
-#define BTE2_WD_DECL
-#define BTE2_WD_POLL(kind, a, b, c, d)
-#endif
-__device__ __forceinline__ void mbar_wait(uint64_t *b, unsigned parity, int tag = 0, int t = 0, int u = 0) {
-  BTE2_WD_DECL;
-  while (!mbar_try(b, parity)) { BTE2_WD_POLL("mbar", tag, t, u, (int)parity) }
+// The wait loop lives inside ONE asm statement (a C++ loop around try_wait is a divergent loop for the compiler).
+__device__ __forceinline__ void mbar_wait(uint64_t *b, unsigned parity) {
+  asm volatile(
+      "{\n.reg .pred P1;\nLAB_WAIT:\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n@P1 bra DONE;\nbra LAB_WAIT;\nDONE:\n}" ::"r"(smem_u32(b)),
+      "r"(parity)
+      : "memory");
 }
 // 1-D bulk copies (TMA).  Loads complete on an mbarrier; stores / reductions are tracked in bulk groups.
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar) {
@@ -265,13 +258,16 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
   constexpr int CP = SM::CP, NCH = SM::NCH, R = D + 1, NBM = BTE2_NBMAX(T);
   typedef Bte2Chunk<T> Ch;
   const unsigned FULL = 0xffffffffu;
-  const int J = threadIdx.x & 31, K = __shfl_sync(FULL, (int)(threadIdx.x >> 5), 0);   // K: warp-uniform for the compiler
+  const int J = threadIdx.x & 31, K = threadIdx.x >> 5;
   const Bte2Oct &O = P.oct[un.oct];
-  const int ty = un.ty, tz = un.tz, b0 = un.b0;
+  const int ty = un.ty, tz = un.tz;
+  // first band of the unit = band group of this CTA = blockIdx.y: only such values stay on the uniform datapath in
+  // this kernel (and the coefficient addressing with them)
+  const int b0 = (int)blockIdx.y * NBM;
   const int jp0 = ty * 64 + 2 * J, kp0 = tz * 2 * W + 2 * K;
   // ny and nz are even on this path (host check): a patch is valid or invalid as a whole, and the last
   // valid row of a tile is always the jj = 1 / kk = 1 row of lane Jl / warp Kl
-  if (kp0 >= P.nz) return;                             // warp without rows (ragged last z tile, two-layer 2-D slabs)
+  if (__all_sync(FULL, kp0 >= P.nz)) return;           // warp without rows (ragged last z tile, two-layer 2-D slabs)
   const bool vthread = jp0 < P.ny;
   const int Jl = (min(P.ny, (ty + 1) * 64) - 1 - ty * 64) >> 1, Kl = (min(P.nz, (tz + 1) * 2 * W) - 1 - tz * 2 * W) >> 1;
   const int ulast = P.nx - 1 + Jl;                     // last local step with an active lane
@@ -317,8 +313,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
       if (peek - ebase > seen) { seen = peek - ebase; sawnew = true; }
       if (seen < need) {
         int v;
-        BTE2_WD_DECL;
-        while ((v = ld_acquire_gpu(P.prog + mydep) - ebase) < need) { __nanosleep(64); BTE2_WD_POLL("dep", unit, mydep, need, v) }
+        while ((v = ld_acquire_gpu(P.prog + mydep) - ebase) < need) __nanosleep(64);
         seen = v; sawnew = true;
       }
     }
@@ -497,7 +492,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
 #pragma unroll
         for (int q = 0; q < 4; ++q) m[a][b][q] = mk2((T)0, (T)0);
 
-    mbar_wait(&BR->full[rb][K], fph, 1, tau, unit);    // the rows of this step have landed
+    mbar_wait(&BR->full[rb][K], fph);                  // the rows of this step have landed
     Bte2Pair<T> in[2][2];
 #pragma unroll
     for (int kk = 0; kk < 2; ++kk)
@@ -523,8 +518,8 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     Ch *__restrict__ zwr = &S->zex[zout][K][0][0][0][J];
     // neighbour-only synchronisation: warp K-1 has written its rows of this step; warp K+1 has read the buffer
     // this step overwrites (written two of its uses ago)
-    if (K > 0) mbar_wait(&BR->zfull[zin][K - 1], (nf >> 1) & 1u, 2, tau, unit);
-    if (feeds && nd >= 2u) mbar_wait(&BR->zempty[zout][K], ((nd >> 1) & 1u) ^ 1u, 3, tau, unit);
+    if (K > 0) mbar_wait(&BR->zfull[zin][K - 1], (nf >> 1) & 1u);
+    if (feeds && nd >= 2u) mbar_wait(&BR->zempty[zout][K], ((nd >> 1) & 1u) ^ 1u);
 
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
@@ -685,11 +680,32 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
   }
 }
 
+template <typename T, int NB, int W, bool MASKED>
+__device__ __forceinline__ void bte2_run_group(const Bte2Dev &P, const Bte2Coefs<T> &CF, unsigned char *smem_raw,
+                                               Bte2Bars<W> *bars, int *s_unit) {
+  constexpr int D = BTE2_DIST(W, T);
+  const int g = blockIdx.y;
+  unsigned nf = 0, nd = 0;                             // this warp's barrier use counters (see Bte2Bars)
+  for (;;) {
+    __syncthreads();                                   // every warp is done with the previous unit (shared memory is free)
+    if (threadIdx.x == 0) {
+      // groups get CTAs in proportion to their work: CTA (x, y) with x >= cta_count[y] leaves without taking a ticket
+      const int tk = (int)blockIdx.x < P.cta_count[g] ? P.gfirst[g] + atomicAdd(P.ticket + g, 1) : P.gfirst[g + 1];
+      *s_unit = tk < P.gfirst[g + 1] ? P.gorder[tk] : -1;
+    }
+    __syncthreads();
+    const int unit = *s_unit;
+    if (unit < 0) break;
+    const Bte2Unit un = P.units[unit];
+    bte2_run_unit<T, NB, W, D, MASKED>(P, CF, un, smem_raw, bars, unit, nf, nd);
+  }
+}
+
 template <typename T, int W, bool MASKED>
 __global__ void __launch_bounds__(W * 32) bte2_sweep_kernel(const __grid_constant__ Bte2Dev P,
                                                             const __grid_constant__ Bte2Coefs<T> CF) {
   extern __shared__ __align__(128) unsigned char bte2_smem_raw[];
-  constexpr int NBMAX = BTE2_NBMAX(T), D = BTE2_DIST(W, T);
+  constexpr int NBMAX = BTE2_NBMAX(T);
   __shared__ int s_unit;
   __shared__ Bte2Bars<W> s_bars;
   if (threadIdx.x == 0) {
@@ -697,17 +713,8 @@ __global__ void __launch_bounds__(W * 32) bte2_sweep_kernel(const __grid_constan
     for (int i = 0; i < (int)(sizeof(s_bars) / 8); ++i) mbar_init(b + i, 1);
     fence_mbar_init();
   }
-  unsigned nf = 0, nd = 0;                             // this warp's barrier use counters (see Bte2Bars)
-  for (;;) {
-    __syncthreads();                                   // every warp is done with the previous unit (shared memory is free)
-    if (threadIdx.x == 0) s_unit = atomicAdd(P.ticket, 1);
-    __syncthreads();
-    const int unit = s_unit;
-    if (unit >= P.n_units) break;
-    const Bte2Unit un = P.units[unit];
-    if (NBMAX == 2 && un.nb == 2) bte2_run_unit<T, NBMAX, W, D, MASKED>(P, CF, un, bte2_smem_raw, &s_bars, unit, nf, nd);
-    else bte2_run_unit<T, 1, W, D, MASKED>(P, CF, un, bte2_smem_raw, &s_bars, unit, nf, nd);
-  }
+  if (NBMAX == 2 && P.B - (int)blockIdx.y * NBMAX >= 2) bte2_run_group<T, NBMAX, W, MASKED>(P, CF, bte2_smem_raw, &s_bars, &s_unit);
+  else bte2_run_group<T, 1, W, MASKED>(P, CF, bte2_smem_raw, &s_bars, &s_unit);
 }
 
 // ------------------------------------------------------------------ boundary kernels (v2 layouts)
@@ -829,7 +836,7 @@ __global__ void bte2_ghost_kernel(const __grid_constant__ Bte2Dev P) {
     for (int sl = 0; sl < 4; ++sl) H += (double)hp[sl];
     Gi[e] = (T)(H / P.Pi_face[P.iface_info[fid]]);
   }
-  if (gtid == 0) *P.ticket = 0;
+  if (gtid < BTE2_MAXB) P.ticket[gtid] = 0;
 }
 
 // ------------------------------------------------------------------ (c) update + residual, v2 layouts
