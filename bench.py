@@ -28,6 +28,8 @@ SM_COUNT, SM_MAX_HZ = 148, 1.965e9
 # plain-ALU peaks derived from unit counts x max clock: FP32 128 FMA/clk/SM,
 # FP64 64 FMA/clk/SM
 PEAK_TFLOPS = {"f32": SM_COUNT * 128 * 2 * SM_MAX_HZ / 1e12, "f64": SM_COUNT * 64 * 2 * SM_MAX_HZ / 1e12}
+# algorithmic HBM bytes per sweep (cell fields + boundary store read and written once)
+ALGORITHMIC_BYTES = {1: 11.2e6, 2: 17.7e6, 3: 63.6e6, 4: 964e6}
 
 
 def parse():
@@ -39,7 +41,8 @@ def parse():
     ap.add_argument("--precision", choices=["config", "f64", "f32"], default="config")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--converge", action="store_true", help="also report time to eps_T <= 1e-8")
+    ap.add_argument("--no-converge", action="store_true", help="skip the time-to-eps_T<=1e-8 run (part of the metric)")
+    ap.add_argument("--converge", action="store_true", help="(default; kept for compatibility)")
     return ap.parse_args()
 
 
@@ -81,7 +84,8 @@ class ClockSampler:
 
 def ncu_traffic(k, dtype):
     """dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch from the committed ncu --set full
-    capture (profiles/ncu_traffic.json, written from the .ncu-rep by hand; None if there is no capture)."""
+    capture of this configuration (profiles/ncu_traffic.json names the capture and its command; None if there is
+    no capture -- DRAM counters cannot be read without a profiler, so this is the one number that is not live)."""
     try:
         with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
             return json.load(f).get(f"config{k}_{dtype}", {}).get("dram_bytes_per_sweep_launch")
@@ -89,10 +93,19 @@ def ncu_traffic(k, dtype):
         return None
 
 
-def oracle_sample(W, k, budget_s, steps):
+def measured_hbm_gbs():
+    """Driver-measured HBM copy bandwidth (MEASURED_PEAKS.json), else the fallback of B200_PROFILING.md."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json"
+    except (OSError, KeyError, ValueError):
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def oracle_sample(W, k, budget_s, steps, cores=None):
     """Pick the largest replica of config k (same physical size, coarser grid) whose `steps` oracle
-    iterations fit `budget_s` on this host; the oracle runs threaded over bands (bit-identical)."""
-    cores = max(1, min(os.cpu_count() or 1, 15))
+    iterations fit `budget_s` on this host; with cores > 1 the oracle runs threaded over bands (bit-identical)."""
+    cores = max(1, min(os.cpu_count() or 1, 15)) if cores is None else cores
     full = W.config(k)
     grids = [(full.nx, full.ny, full.nz)]
     while max(grids[-1]) > 8:
@@ -106,9 +119,9 @@ def oracle_sample(W, k, budget_s, steps):
     return p, g, cores
 
 
-def time_oracle(W, k, budget_s, steps=1, warmup=0):
+def time_oracle(W, k, budget_s, steps=1, warmup=0, cores=None):
     import oracle
-    p, grid, cores = oracle_sample(W, k, budget_s, steps + warmup)
+    p, grid, cores = oracle_sample(W, k, budget_s, steps + warmup, cores)
     r = oracle.RefSolver(p, threads=cores)
     r.iterate(warmup)
     t0 = time.perf_counter()
@@ -116,7 +129,8 @@ def time_oracle(W, k, budget_s, steps=1, warmup=0):
     dt = time.perf_counter() - t0
     return {"value": p.updates_per_sweep * steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{steps} source iteration(s) of config {k} on a {grid[0]}x{grid[1]}x{grid[2]} replica "
-                      f"({p.updates_per_sweep:.3e} updates each), oracle threaded over bands"}, dt / steps, p
+                      f"({p.updates_per_sweep:.3e} updates each), oracle on {cores} thread(s)"
+                      + (" over bands" if cores > 1 else "")}, dt / steps, p
 
 
 def run_reference(args, W):
@@ -192,6 +206,9 @@ def run_ours(args, W):
     solver = bte.Solver(p, precision=prec, device=dev)
     K, Wm = args.steps, max(args.warmup, 3)
     upd = solver.updates_per_sweep
+    # plain-ALU peak measured in this run (register-only FFMA2 / DFMA chains on every SM), before the timed region
+    import microbench
+    peak_measured, n_sms = microbench.measure_fma_peak(dtype, dev)
 
     # ---- device-resident timing: K iterations in one bte_iterate call (inputs already in HBM)
     solver.iterate(Wm)
@@ -216,17 +233,18 @@ def run_ours(args, W):
     Qsrc = p.Q if p.Q is not None else np.zeros((p.nz, p.ny, p.nx))
     Qh = torch.from_numpy(np.ascontiguousarray(Qsrc, dtype=np.float64)).pin_memory()
     dTh = torch.empty(solver.shape, dtype=torch.float64).pin_memory()
+    qh = torch.empty((3,) + solver.shape, dtype=torch.float64).pin_memory()
     for _ in range(3):
-        solver.solve_host(Qh, 1, reset=False, out=(dTh, None))
+        solver.solve_host(Qh, 1, reset=False, out=(dTh, qh))
     barrier()
     t0 = time.perf_counter()
     for _ in range(K):
-        solver.solve_host(Qh, 1, reset=False, out=(dTh, None))
+        solver.solve_host(Qh, 1, reset=False, out=(dTh, qh))
     barrier()
     e2e_s = R.max(time.perf_counter() - t0)
 
     conv = None
-    if args.converge and rank == 0:
+    if not args.no_converge and rank == 0:
         solver.solve_host(Qh, 0, reset=True, out=(dTh, None))
         torch.cuda.synchronize()
         t0, n = time.perf_counter(), 0
@@ -236,13 +254,21 @@ def run_ours(args, W):
             if solver.residual()[0] <= 1e-8:
                 break
         conv = {"eps_T_target": 1e-8, "iterations": n, "seconds": time.perf_counter() - t0,
-                "eps_T": solver.residual()[0]}
+                "eps_T": solver.residual()[0], "reached": solver.residual()[0] <= 1e-8,
+                "what": "wall time of bte_iterate from dT = 0, bte_residual checked every 25 iterations (cap 20000)"}
 
     if rank == 0:
         sweep_avg_ms = sweep_ms / max(sweep_n, 1)
         achieved = upd * FLOP_PER_UPDATE / (sweep_avg_ms * 1e-3) / 1e12
         peak = PEAK_TFLOPS[dtype]
         info = solver.schedule_info()
+        # both floors of the sweep launch AS BUILT: t_alu = algorithmic flop / derived FMA peak, t_hbm = DRAM bytes the
+        # kernel actually moves (ncu capture of this configuration) / measured HBM copy bandwidth; the larger one binds
+        traffic = ncu_traffic(args.config, dtype)
+        hbm_gbs, hbm_src = measured_hbm_gbs()
+        t_alu_ms = upd * FLOP_PER_UPDATE / (peak * 1e12) * 1e3
+        t_hbm_ms = traffic / (hbm_gbs * 1e9) * 1e3 if traffic else None
+        bound = "hbm" if (t_hbm_ms is not None and t_hbm_ms > t_alu_ms) else "alu"
         line = {"metric": METRIC, "value": world * upd * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
                 "steps": K, "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": dtype, "data": "synthetic",
@@ -254,13 +280,22 @@ def run_ours(args, W):
                            "eps_T_after_timed_steps": eps[0]},
                 "clocks": clocks,
                 "e2e": {"value": world * upd * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": Qh.numel() * 8,
-                        "d2h_bytes_per_step": dTh.numel() * 8,
-                        "what": "bte_solve_host(Q pinned host -> 1 iteration -> dT pinned host) per step"},
+                        "d2h_bytes_per_step": (dTh.numel() + qh.numel()) * 8,
+                        "what": "bte_solve_host(Q pinned host -> 1 iteration -> dT and q pinned host) per step"},
                 "gpu_launches": solver.launches_per_iteration * K,
-                "roofline": {"bound": "alu", "kernel": "bte2_sweep_kernel" if solver.kernel_path == 2 else "bte_sweep_kernel",
+                "roofline": {"bound": bound, "kernel": "bte2_sweep_kernel" if solver.kernel_path == 2 else "bte_sweep_kernel",
                              "achieved": achieved, "peak": peak,
-                             "unit": "TFLOP/s", "frac": achieved / peak, "traffic": ncu_traffic(args.config, dtype),
+                             "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
                              "peak_source": "derived: 148 SMs x %d FMA/clk x 2 x 1.965 GHz (DESIGN.md)" % (128 if dtype == "f32" else 64),
+                             "peak_measured": peak_measured, "frac_of_measured": achieved / peak_measured,
+                             "peak_measured_source": "microbench/fma_peak.cu in this run: register-only %s chains, %d SMs, "
+                                                     "SM clock %s MHz during the timed region" %
+                                                     ("FFMA2" if dtype == "f32" else "DFMA", n_sms, clocks.get("sm_mhz")),
+                             "t_alu_ms": t_alu_ms, "t_hbm_ms": t_hbm_ms,
+                             "hbm": {"achieved_gbs": traffic / (sweep_avg_ms * 1e-3) / 1e9 if traffic else None,
+                                     "peak_gbs": hbm_gbs, "peak_source": hbm_src,
+                                     "frac": traffic / (sweep_avg_ms * 1e-3) / 1e9 / hbm_gbs if traffic else None,
+                                     "algorithmic_bytes": ALGORITHMIC_BYTES.get(args.config)},
                              "ms_per_launch": sweep_avg_ms, "launches_timed": sweep_n,
                              "share_of_step": sweep_ms / ms if ms > 0 else None,
                              "wavefront_occupancy": upd / info["thread_slot_updates"]},
@@ -268,7 +303,9 @@ def run_ours(args, W):
         if conv:
             line["time_to_1e-8"] = conv
         if not args.no_cpu_baseline and world == 1:
-            line["cpu_baseline"] = time_oracle(W, args.config, budget_s=20.0, steps=1)[0]
+            # the oracle as it stands: single thread first, then threaded over bands
+            line["cpu_baseline"] = time_oracle(W, args.config, budget_s=12.0, steps=1, cores=1)[0]
+            line["cpu_baseline_threads"] = time_oracle(W, args.config, budget_s=12.0, steps=1)[0]
         print(json.dumps(line), flush=True)
     R.close()
 

@@ -143,11 +143,13 @@ int32_t bte_last_cuda_error(void);
  * already created are not affected).  The library never reads the environment.  value 0 = default.
  *   BTE_OPT_FORCE_GENERIC   1: use the generic kernels for every problem
  *   BTE_OPT_WARPS           2 | 4 | 8: warps per CTA of the fast path (default: by nz)
- *   BTE_OPT_PUBLISH_PERIOD  2 | 4 | 8 | 16 | 32: steps between progress publications of a warp (default 8; 4 if nx <= 96)
+ *   BTE_OPT_PUBLISH_PERIOD  4 | 8 | 16 | 32: steps between progress publications of a unit (default 8; 4 if nx <= 96)
  *   BTE_OPT_START_SLACK     1..256: extra steps a unit lets the units it follows get ahead before it starts
+ *   BTE_OPT_SCHEDULE        1: ticket order = band groups of one (tile, octant) consecutively instead of the simulated
+ *                           list schedule (experiment on L2 reuse; same results, different timing)
  * Returns BTE_ERR_INVALID_ARG for an unknown option. */
 typedef enum { BTE_OPT_FORCE_GENERIC = 0, BTE_OPT_WARPS = 1, BTE_OPT_PUBLISH_PERIOD = 2, BTE_OPT_START_SLACK = 3,
-               BTE_OPT_COUNT_ = 4 } bte_option;
+               BTE_OPT_SCHEDULE = 4, BTE_OPT_COUNT_ = 5 } bte_option;
 bte_status bte_set_option(int32_t option, int32_t value);
 
 #ifdef __cplusplus

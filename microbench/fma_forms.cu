@@ -1,5 +1,5 @@
 // Microbenchmark (not part of the library): FMA-pipe rate of the FFMA / FFMA2 operand forms the sweep uses, on sm_100a.
-// Build + run:  nvcc -gencode arch=compute_100a,code=sm_100a -O3 -std=c++17 -o /tmp/fma_forms microbench_fma_forms.cu && /tmp/fma_forms
+// Build + run:  nvcc -gencode arch=compute_100a,code=sm_100a -O3 -std=c++17 -o /tmp/fma_forms microbench/fma_forms.cu && /tmp/fma_forms
 // Result on B200: profiles/r01_fma_forms_microbench.txt (every form with a uniform-register coefficient runs at the full 128 FMA/clk/SM).
 #include <cstdio>
 #include <cuda_runtime.h>

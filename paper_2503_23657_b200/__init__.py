@@ -114,7 +114,7 @@ def lib():
     return _lib
 
 
-OPTIONS = {"force_generic": 0, "warps": 1, "publish_period": 2, "start_slack": 3}
+OPTIONS = {"force_generic": 0, "warps": 1, "publish_period": 2, "start_slack": 3, "schedule": 4}
 
 
 def bte_set_option(name, value) -> None:

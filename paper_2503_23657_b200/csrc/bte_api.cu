@@ -54,7 +54,6 @@ struct Plan {
   std::vector<uint32_t> codeP[4];
   Bte2Dev d2{};
   std::vector<Bte2Unit> units2;
-  std::vector<int32_t> gorder2;          // unit ids in ticket order, band group after band group
   Bte2Coefs<float> cf32{};
   Bte2Coefs<double> cf64{};
   size_t smem2 = 0;
@@ -254,7 +253,7 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
       pl.item_coef[(size_t)o * max_items + b * O.nchunk + c] = off;
     }
   }
-  if (pl.coef.size() * tsz > BTE_CONST_BYTES) return BTE_ERR_UNSUPPORTED;
+  const bool const_overflow = pl.coef.size() * tsz > BTE_CONST_BYTES;   // only the generic path keeps the table in c_coef
 
   // ---- work units in ticket (topological) order: key = item + ty + tz
   struct Key { int key, o, item, ty, tz; };
@@ -312,20 +311,20 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
     }
   }
   pl.v2 = v2;
+  if (!v2 && const_overflow) return BTE_ERR_UNSUPPORTED;
   if (v2) {
     Bte2Dev &d = pl.d2;
     int W = p->nz >= 48 ? 8 : (p->nz <= 4 ? 2 : 4);   // 2 warps: thin slabs (the two-layer form of 2-D problems)
     { const int w = g_opt[BTE_OPT_WARPS].load(); if (w == 2 || w == 4 || w == 8) W = w; }
     d.nx = p->nx; d.ny = p->ny; d.nz = p->nz; d.B = B; d.W = W;
     d.nty = (p->ny + 63) / 64; d.ntz = (p->nz + 2 * W - 1) / (2 * W); d.NU = p->nx + 31;
-    d.nsteps = p->nx + 32 + W - 1;                   // nx + 32 local steps per warp, warp K one step behind warp K-1
-    d.pub_mask = (p->nx <= 96 ? BTE2_PUB / 2 : BTE2_PUB) - 1; d.slack = 0;   // short rows: publish progress twice as often (measured)
-    { const int v = g_opt[BTE_OPT_PUBLISH_PERIOD].load(); if (v == 2 || v == 4 || v == 8 || v == 16 || v == 32) d.pub_mask = v - 1; }
+    d.nsteps = p->nx + 31 + W - 1;
+    d.pub_mask = (p->nx <= 96 ? BTE2_PUB / 2 : BTE2_PUB) - 1; d.slack = BTE2_SLACK;   // short rows: publish progress twice as often (measured)
+    { const int v = g_opt[BTE_OPT_PUBLISH_PERIOD].load(); if (v == 4 || v == 8 || v == 16 || v == 32) d.pub_mask = v - 1; }
     { const int v = g_opt[BTE_OPT_START_SLACK].load(); if (v > 0 && v <= 256) d.slack = v; }
     d.NS = (int64_t)p->nz * d.nty * d.NU * 64;
     d.ncell = N; d.src_mod = N; d.inv_sumCtau = dv.inv_sumCtau;
     const int NBmax = dv.fp32 ? 2 : 1, G = (B + NBmax - 1) / NBmax;
-    d.G = G;
     for (int b = 0; b < B; ++b) {
       const double *blk = pl.coef.data() + pl.item_coef[b];
       for (int q = 0; q < BTE2_P; ++q) {
@@ -374,8 +373,8 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
     d.n_units = (int32_t)pl.units2.size();
     const size_t nch = BTE2_P * tsz / 16;
     pl.x2_chunks = (size_t)d.ntz * d.nty * B * W * 2 * 2 * nch * 32;
-    pl.y2_slot = (size_t)d.ntz * G * W * d.nx * NBmax * 2 * nch;      // rows of whole band groups (bte_sweep2.cuh layouts)
-    pl.z2_slot = (size_t)d.nty * G * d.NU * NBmax * 2 * nch * 32;
+    pl.y2_slot = (size_t)d.ntz * B * W * d.nx * 2 * nch;
+    pl.z2_slot = (size_t)d.nty * B * d.NU * 2 * nch * 32;
     pl.y2_chunks = (size_t)(d.nty + 2) * pl.y2_slot;
     pl.z2_chunks = (size_t)(d.ntz + 2) * pl.z2_slot;
     int64_t off = 0;
@@ -435,7 +434,6 @@ size_t bind(Plan &pl, unsigned char *ws) {
     Bte2Dev &d = pl.d2;
     const size_t NS2 = (size_t)d.NS;
     d.units = (const Bte2Unit *)take(pl.units2.size() * sizeof(Bte2Unit));
-    d.gorder = (const int32_t *)take(pl.units2.size() * 4);
     if (pl.masked2) {
       d.code = dv.code;
       for (int c = 0; c < 4; ++c) d.codeP[c] = (const uint32_t *)take((size_t)(dv.nz / 2) * d.nty * d.NU * 32 * 4);
@@ -449,7 +447,7 @@ size_t bind(Plan &pl, unsigned char *ws) {
     pl.state_begin = off;
     d.Gi = d.n_iface ? take((size_t)d.n_iface * d.B * tsz) : nullptr;
     d.Hd = (d.n_iface && d.iface_type == 1) ? take((size_t)6 * N * d.B * 4 * tsz) : nullptr;
-    d.prog = (int32_t *)take((size_t)d.n_units * d.W * 4);
+    d.prog = (int32_t *)take((size_t)d.n_units * 4);
     d.ticket = (int32_t *)take(256);
     dv.red = (double *)take((size_t)(4 * dv.n_red_blocks + 4) * 8);
     dv.dT = (double *)take(N * 8);
@@ -495,80 +493,70 @@ size_t bind(Plan &pl, unsigned char *ws) {
   return off;
 }
 
-// Schedule of the fast path.  Every CTA serves one band group (bte_sweep2.cuh): the `slots` resident CTAs are shared out
-// to the groups in proportion to their work (a group of one band costs half a group of two), and each group's ticket
-// order is the start order of a list schedule simulated with these per-group CTA pools: a unit may start once every
-// unit it follows is `lag` steps ahead, so that the per-step dependency polls of the kernel (which stay in place for
-// correctness) almost never have to wait, and the G groups work on the same tile at the same time (L2 reuse of the
-// cell inputs and of the accumulator rows).  Deadlock-free for any slots >= G: group g only follows group g - 1 and
-// earlier units of its own list.
+// Ticket order of the fast path = start order of a list schedule simulated on `slots` resident CTAs:
+// a unit may start once every unit it follows is lag + BTE2_SLACK steps ahead, so that the per-step
+// dependency polls of the kernel (which stay in place for correctness) almost never have to wait.
 void order_units2(Plan &pl, int slots) {
   std::vector<Bte2Unit> &U = pl.units2;
-  Bte2Dev &d = pl.d2;
-  const int n = (int)U.size(), W = d.W, nsteps = d.nsteps, G = d.G;
+  const int n = (int)U.size(), W = pl.d2.W, nsteps = pl.d2.nsteps;
   const int NBmax = pl.dev.fp32 ? 2 : 1;
-  // CTAs per group
-  std::vector<int> ng(G, 0), cnt(G, 1);
-  std::vector<double> wg(G, 1.0);
-  for (int u = 0; u < n; ++u) { ++ng[U[u].g]; wg[U[u].g] = (double)U[u].nb / NBmax; }
-  slots = std::max(slots, G);
-  double wsum = 0;
-  for (int g = 0; g < G; ++g) wsum += wg[g];
-  int used = 0;
-  for (int g = 0; g < G; ++g) { cnt[g] = std::max(1, std::min(ng[g], (int)std::floor(slots * wg[g] / wsum))); used += cnt[g]; }
-  for (;;) {   // hand the remaining CTAs to the group with the longest queue per CTA
-    int best = -1; double load = 0;
-    for (int g = 0; g < G; ++g) if (cnt[g] < ng[g] && ng[g] * wg[g] / cnt[g] > load) { load = ng[g] * wg[g] / cnt[g]; best = g; }
-    if (best < 0 || used >= slots) break;
-    ++cnt[best]; ++used;
-  }
-  for (int g = 0; g < BTE2_MAXB; ++g) d.cta_count[g] = g < G ? cnt[g] : 0;
-  // list schedule
   std::vector<double> start(n, -1.0), steptime(n);
-  std::vector<int> ndep(n, 0);
+  std::vector<int> ndep(n, 0), order;
   std::vector<std::vector<int>> succ(n);
   for (int u = 0; u < n; ++u) {
     steptime[u] = (double)U[u].nb / NBmax;
     const int deps[3] = {U[u].dep_y, U[u].dep_z, U[u].dep_prev};
-    for (int dd : deps) if (dd >= 0) { ++ndep[u]; succ[dd].push_back(u); }
+    for (int d : deps) if (d >= 0) { ++ndep[u]; succ[d].push_back(u); }
   }
-  const int D = pl.dev.fp32 ? BTE2_DIST(W, float) : BTE2_DIST(W, double);
   auto allowed = [&](int u) {
     const int deps[3] = {U[u].dep_y, U[u].dep_z, U[u].dep_prev};
-    // steps the followed unit must be ahead: y outflow lag + prefetch distance; z: its last warp trails its first by W - 1
-    const int lag[3] = {BTE2_YLAG + D, W + D, 1};
+    const int lag[3] = {33, W + 1, 1};
     double a = 0;
     for (int k = 0; k < 3; ++k)
-      if (deps[k] >= 0) a = std::max(a, start[deps[k]] + (lag[k] + d.slack + d.pub_mask + 2) * steptime[deps[k]]);
+      if (deps[k] >= 0) a = std::max(a, start[deps[k]] + (lag[k] + (pl.dev.fp32 ? BTE2_DIST(W, float) : BTE2_DIST(W, double)) + pl.d2.slack + pl.d2.pub_mask + 1) * steptime[deps[k]]);
     return a;
   };
   typedef std::pair<double, int> Key;
-  typedef std::priority_queue<Key, std::vector<Key>, std::greater<Key>> Heap;
-  std::vector<Heap> ready(G), freeslot(G);
-  for (int g = 0; g < G; ++g) for (int k = 0; k < cnt[g]; ++k) freeslot[g].push({0.0, k});
-  for (int u = 0; u < n; ++u) if (ndep[u] == 0) ready[U[u].g].push({0.0, u});
-  std::vector<std::vector<int>> order(G);
-  for (int done = 0; done < n; ++done) {
-    int bg = -1; double bt = 0;
-    for (int g = 0; g < G; ++g) {
-      if (ready[g].empty()) continue;
-      const double t = std::max(ready[g].top().first, freeslot[g].top().first);
-      if (bg < 0 || t < bt) { bg = g; bt = t; }
-    }
-    if (bg < 0) break;                    // cannot happen: the dependency graph is acyclic
-    const int u = ready[bg].top().second; ready[bg].pop();
-    const Key f = freeslot[bg].top(); freeslot[bg].pop();
-    start[u] = bt;
-    freeslot[bg].push({bt + nsteps * steptime[u], f.second});
-    order[bg].push_back(u);
-    for (int v : succ[u]) if (--ndep[v] == 0) ready[U[v].g].push({allowed(v), v});
+  std::priority_queue<Key, std::vector<Key>, std::greater<Key>> ready, freeslot;
+  for (int u = 0; u < n; ++u) if (ndep[u] == 0) ready.push({0.0, u});
+  for (int k = 0; k < std::max(slots, 1); ++k) freeslot.push({0.0, k});
+  order.reserve(n);
+  if (g_opt[BTE_OPT_SCHEDULE].load() == 1) {
+    // "gang" order (experiment): the band groups of one (tile, octant) take consecutive tickets, tiles in (ty, tz) order
+    // -- topological, and group g + 1 trails group g on the same tile by the publication period (L2 reuse of the
+    // accumulator rows and cell inputs of the tile)
+    std::vector<int> idx(n);
+    for (int u = 0; u < n; ++u) idx[u] = u;
+    std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) {
+      const Bte2Unit &A = U[a], &B = U[b];
+      if (A.ty != B.ty) return A.ty < B.ty;
+      if (A.tz != B.tz) return A.tz < B.tz;
+      if (A.oct != B.oct) return A.oct < B.oct;
+      return A.g < B.g;
+    });
+    order = idx;
+    while (!ready.empty()) ready.pop();
   }
-  pl.gorder2.clear();
-  for (int g = 0; g < G; ++g) {
-    d.gfirst[g] = (int32_t)pl.gorder2.size();
-    pl.gorder2.insert(pl.gorder2.end(), order[g].begin(), order[g].end());
+  while (!ready.empty()) {
+    const Key f = freeslot.top(); freeslot.pop();
+    const Key r = ready.top(); ready.pop();
+    const int u = r.second;
+    start[u] = std::max(f.first, r.first);
+    freeslot.push({start[u] + nsteps * steptime[u], f.second});
+    order.push_back(u);
+    for (int v : succ[u]) if (--ndep[v] == 0) ready.push({allowed(v), v});
   }
-  for (int g = G; g <= BTE2_MAXB; ++g) d.gfirst[g] = (int32_t)pl.gorder2.size();
+  std::vector<int> newid(n);
+  for (int k = 0; k < n; ++k) newid[order[k]] = k;
+  std::vector<Bte2Unit> out(n);
+  for (int k = 0; k < n; ++k) {
+    Bte2Unit x = U[order[k]];
+    if (x.dep_y >= 0) x.dep_y = newid[x.dep_y];
+    if (x.dep_z >= 0) x.dep_z = newid[x.dep_z];
+    if (x.dep_prev >= 0) x.dep_prev = newid[x.dep_prev];
+    out[k] = x;
+  }
+  U.swap(out);
 }
 
 }  // namespace
@@ -617,11 +605,8 @@ bte_status skew(bte_solver *h, const double *src, double scale, int which, cudaS
 
 template <typename T, int W>
 void launch_sweep2(bte_solver *h, const Bte2Coefs<T> &cf, cudaStream_t st) {
-  int cmax = 1;
-  for (int g = 0; g < h->pl.d2.G; ++g) cmax = std::max(cmax, h->pl.d2.cta_count[g]);
-  const dim3 grid((unsigned)cmax, (unsigned)h->pl.d2.G);   // CTA (x, y): band group y; it leaves at once if x >= cta_count[y]
-  if (h->pl.masked2) bte2_sweep_kernel<T, W, true><<<grid, W * 32, h->pl.smem2, st>>>(h->pl.d2, cf);
-  else bte2_sweep_kernel<T, W, false><<<grid, W * 32, h->pl.smem2, st>>>(h->pl.d2, cf);
+  if (h->pl.masked2) bte2_sweep_kernel<T, W, true><<<h->sweep_grid, W * 32, h->pl.smem2, st>>>(h->pl.d2, cf);
+  else bte2_sweep_kernel<T, W, false><<<h->sweep_grid, W * 32, h->pl.smem2, st>>>(h->pl.d2, cf);
 }
 
 template <typename T>
@@ -631,7 +616,7 @@ bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t
   const int bgrid = h->num_sms * 8;
   for (int it = 0; it < n; ++it) {
     const int ep = (int)(h->iters % 30000) + 1;
-    if (ep == 1 && h->iters > 0) CK(cudaMemsetAsync(d.prog, 0, (size_t)d.n_units * d.W * 4, st));
+    if (ep == 1 && h->iters > 0) CK(cudaMemsetAsync(d.prog, 0, (size_t)d.n_units * 4, st));
     d.epoch = ep;
     d.fill_iso = h->iters == 0;
     {   // ghost planes to fill: diffuse faces every iteration, isothermal faces once (specular / periodic: none)
@@ -676,6 +661,7 @@ bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t
     bte2_update_kernel<T><<<pl.dev.n_red_blocks, 256, 0, st>>>(d);
     bte_final_kernel<<<1, 256, 0, st>>>(pl.dev);
     h->iters += 1;
+    if (it == 0) CK(cudaGetLastError());   // a bad launch configuration shows up at once, not after n queued iterations
   }
   CK(cudaGetLastError());
   return BTE_OK;
@@ -684,7 +670,7 @@ bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t
 template <typename T, int W>
 bte_status setup_sweep2_W(bte_solver *h) {
   Plan &pl = h->pl;
-  pl.smem2 = sizeof(Bte2Smem<T, BTE2_NBMAX(T), W, BTE2_DIST(W, T)>);
+  pl.smem2 = sizeof(Bte2Smem<T, sizeof(T) == 4 ? 2 : 1, W, BTE2_DIST(W, T)>);
   int occ = 0;
   if (pl.masked2) {
     CK(cudaFuncSetAttribute(bte2_sweep_kernel<T, W, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem2));
@@ -694,7 +680,7 @@ bte_status setup_sweep2_W(bte_solver *h) {
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bte2_sweep_kernel<T, W, false>, W * 32, pl.smem2));
   }
   if (occ < 1) { g_last_cuda.store((int)cudaErrorLaunchOutOfResources); return BTE_ERR_CUDA; }
-  h->sweep_grid = std::max(pl.d2.G, h->num_sms * occ);   // resident CTA budget (order_units2 shares it out to the band groups)
+  h->sweep_grid = (int)std::min<int64_t>(pl.d2.n_units, (int64_t)h->num_sms * occ);
   pl.nthreads = W * 32;
   return BTE_OK;
 }
@@ -720,6 +706,7 @@ bte_status iterate_T(bte_solver *h, int n, cudaStream_t st) {
     bte_update_kernel<T><<<dv.n_red_blocks, 256, 0, st>>>(dv);
     bte_final_kernel<<<1, 256, 0, st>>>(dv);
     h->iters += 1;
+    if (it == 0) CK(cudaGetLastError());
   }
   CK(cudaGetLastError());
   return BTE_OK;
@@ -774,9 +761,6 @@ bte_status bte_create(const bte_problem *p, void *d_workspace, size_t bytes, voi
   if (pl.v2) {
     order_units2(pl, h->sweep_grid);
     CKD(cudaMemcpyAsync((void *)pl.d2.units, pl.units2.data(), pl.units2.size() * sizeof(Bte2Unit), cudaMemcpyHostToDevice, s));
-    CKD(cudaMemcpyAsync((void *)pl.d2.gorder, pl.gorder2.data(), pl.gorder2.size() * 4, cudaMemcpyHostToDevice, s));
-    h->sweep_grid = 0;
-    for (int g = 0; g < pl.d2.G; ++g) h->sweep_grid += pl.d2.cta_count[g];   // CTAs that take tickets
     if (pl.masked2) {
       for (int c = 0; c < 4; ++c)
         CKD(cudaMemcpyAsync((void *)pl.d2.codeP[c], pl.codeP[c].data(), pl.codeP[c].size() * 4, cudaMemcpyHostToDevice, s));
@@ -940,22 +924,6 @@ bte_status bte_plan_info(const bte_problem *p, int32_t resident_ctas, int64_t ou
   }
   order_units2(pl, std::max(resident_ctas, 1));
   bool topo = true, same = true;
-  {   // every group's ticket list holds exactly its units, each after the units of the same group it follows
-    std::vector<int> pos(pl.units2.size(), -1);
-    for (size_t k = 0; k < pl.gorder2.size(); ++k) pos[pl.gorder2[k]] = (int)k;
-    int ctas = 0;
-    for (int g = 0; g < pl.d2.G; ++g) {
-      ctas += pl.d2.cta_count[g];
-      topo = topo && pl.d2.cta_count[g] >= 1;
-      for (int k = pl.d2.gfirst[g]; k < pl.d2.gfirst[g + 1]; ++k) topo = topo && pl.units2[pl.gorder2[k]].g == g;
-    }
-    topo = topo && pl.gorder2.size() == pl.units2.size() && ctas <= std::max(resident_ctas, pl.d2.G);
-    for (size_t u = 0; u < pl.units2.size(); ++u) {
-      const Bte2Unit &U = pl.units2[u];
-      topo = topo && pos[u] >= 0;
-      for (int d : {U.dep_y, U.dep_z}) if (d >= 0) topo = topo && pos[d] < pos[u];
-    }
-  }
   for (size_t u = 0; u < pl.units2.size(); ++u) {
     const Bte2Unit &U = pl.units2[u];
     for (int d : {U.dep_y, U.dep_z, U.dep_prev}) topo = topo && d < (int)u;

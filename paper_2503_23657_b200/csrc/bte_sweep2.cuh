@@ -3,12 +3,11 @@
 //
 // Mapping.  One CTA = W warps sweeps one tile = 64 (y') x 2W (z') rows along x' for one octant and
 // one band group (NB = 1 or 2 bands x 16 directions).  Thread (J = lane, K = warp) owns the 2x2
-// row patch j' = 64 ty + 2J + {0,1}, k' = 2W tz + 2K + {0,1}; at its LOCAL step tau warp K works on
-// i' = tau - J (lane-skewed wavefront), and warp K runs its step tau after warp K-1 has run the same
-// step (warp-skewed wavefront), so that
+// row patch j' = 64 ty + 2J + {0,1}, k' = 2W tz + 2K + {0,1} and marches i' = t - J - K
+// (lane/warp-skewed wavefront), so that
 //   x-upwind  = its own register (carry),
 //   y-upwind  = its own patch row jj=0, or lane J-1's jj=1 row of the previous step (one SHFL),
-//   z-upwind  = its own patch row kk=0, or warp K-1's kk=1 row of the same step (16-byte
+//   z-upwind  = its own patch row kk=0, or warp K-1's kk=1 row of the previous step (16-byte
 //               shared-memory exchange, double buffered),
 // i.e. 64 NB updates per thread and step need 32 NB shuffles and 16 NB 16-byte LDS/STS.  The
 // recurrence/moment coefficients are warp-uniform kernel parameters (constant bank -> uniform
@@ -16,25 +15,10 @@
 // The (band x direction) intensity lives in registers only; tile faces go through L2-resident
 // planes (hand-off to the downstream tile, or the lagged boundary store at box faces).
 //
-// Plumbing.  Everything a warp needs for one step is ONE contiguous row per array in global memory
-// (cell inputs 1 KB, y inflow 256 B, z inflow 8 KB, moments 2 KB, ...), moved by 1-D bulk copies (TMA)
-// that lane 0 of the warp issues: loads D steps ahead onto an mbarrier, stores from shared-memory
-// staging, and the moment sums of a band group are ADDED to the octant accumulator by the L2
-// (cp.reduce.async.bulk .add), so the accumulator is never read back by the sweep.  There is no
-// CTA-wide barrier in the step loop: warp K waits for warp K-1's rows (mbarrier zfull) and for warp
-// K+1 to have released the buffer it overwrites (mbarrier zempty); the warps of a CTA drift against
-// each other, so one warp's memory-side work overlaps the other warps' arithmetic.
-//
-// Scheduling.  Every persistent CTA serves ONE band group for the whole launch (the group is blockIdx.y) and takes tickets from that group's unit list, which is in topological order.
-// So the band index is a function of blockIdx alone: the compiler keeps the coefficient addressing on
-// the uniform datapath (measured on the SASS: values that come from memory, from warp votes or even
-// from kernel parameters do not qualify inside this kernel, and the FFMA2s then take three vector
-// operands and a constant load each), and the CTAs of the G groups sweep the same tile at the same time,
-// each a few steps behind the previous group, so the cell inputs and the accumulator rows of a tile
-// stay in the L2 between the groups.  Dependencies between tiles are tracked per WARP and per STEP,
-// not per tile: every warp publishes its step count (release store) every BTE2_PUB steps, and the
-// downstream tile in y / z (and the next band group on the same tile, whose additions to the
-// accumulator must come after this one's) stays behind it.
+// Scheduling.  Persistent CTAs take tickets in a topological unit order.  Dependencies between
+// tiles are tracked per STEP, not per tile: every unit publishes its step count (release store)
+// every BTE2_PUB steps, and the downstream tile in y / z (and the previous band group on the same
+// tile, which owns the moment accumulator before it) only has to stay 32 / W / 1 steps behind.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -45,9 +29,18 @@
 #define BTE2_P 16         // directions per octant
 #define BTE2_MAXB 16      // bands in the parameter table
 #define BTE2_PUB 8        // progress is published every PUB steps
-#define BTE2_DIST(W, T) (((W) >= 8 && sizeof(T) == 8) ? 1 : 2)   // bulk-load prefetch distance in steps (shared-memory budget)
-#define BTE2_NBMAX(T) (sizeof(T) == 4 ? 2 : 1)                    // bands per unit
-#define BTE2_YLAG 33      // a warp reads the y outflow of cell i' of the upstream tile: emitted at upstream step i' + 32
+#define BTE2_DIST(W, T) (sizeof(T) == 4 ? 2 : 1)   // cp.async prefetch distance in steps (shared-memory budget; >= 1 + BTE2_MDIST)
+#define BTE2_MDIST(T) (sizeof(T) == 4 ? 1 : 0)   // same for the moment accumulator (fp64: fetched in the step that adds to it)
+#ifndef BTE2_SPLITBAR
+#define BTE2_SPLITBAR 1   // 0: plain __syncthreads per step (config 4 sweep 5.23 ms instead of 4.89 ms)
+#endif
+#define BTE2_SLACK 0      // extra steps a unit lets the units it follows get ahead before it starts
+// timing experiments only (-DBTE2_ENABLE_DBG + env BTE_V2_DBG): the product build compiles the switches out
+#ifdef BTE2_ENABLE_DBG
+#define BTE2_DBGBIT(P, bit) ((P).dbg & (bit))
+#else
+#define BTE2_DBGBIT(P, bit) 0
+#endif
 
 template <typename T> struct alignas(16) Bte2Coefs {   // kernel parameter (constant bank 0)
   T k[BTE2_MAXB][8][BTE2_P];   // [band][inv, ax, ay, az, w/tau, v w|sx|, v w|sy|, v w|sz|][direction]
@@ -79,16 +72,13 @@ struct Bte2Oct {
 struct Bte2Dev {
   int32_t nx, ny, nz, B;
   int32_t W, nty, ntz, NU;          // warps per CTA; tiles along y', z'; nx + 31
-  int32_t nsteps, n_units, epoch, G;   // nsteps: local steps of a warp (nx + 32); G: band groups
+  int32_t nsteps, n_units, epoch, dbg;   // dbg: timing experiments only (BTE_V2_DBG), 0 in production
   int64_t NS;                       // nz * nty * NU * 64
   void *dTQ[4];                     // T2 [NS]: (dT, Q / sum C) per x/y-flip class
   Bte2Oct oct[8];
   const Bte2Unit *units;
-  const int32_t *gorder;            // unit ids in ticket order, group after group: group g owns [gfirst[g], gfirst[g+1])
-  int32_t gfirst[BTE2_MAXB + 1];
-  int32_t cta_count[BTE2_MAXB];     // grid = (max cta_count, G): CTA (x, y) serves band group y; it leaves at once if x >= cta_count[y]
-  int32_t *prog;                    // [n_units][W] epoch << 16 | steps published by warp K of the unit
-  int32_t *ticket;                  // [BTE2_MAXB] one ticket counter per band group
+  int32_t *prog;                    // [n_units] epoch << 16 | steps published
+  int32_t *ticket;
   // boundary conditions (box faces x-,x+,y-,y+,z-,z+) and the update kernel
   int32_t face_type[6];
   double face_e0[6][BTE2_MAXB];     // isothermal inflow C_b dT_w / 4pi (Eq. 5)
@@ -97,7 +87,7 @@ struct Bte2Dev {
   void *Gf;                         // T diffuse inflow [f][b][tb][ta]
   int64_t gf_off[7];                // offsets of the 6 faces in Gf, [6] = total
   double *dT, *q, *qmag, *red;      // fp64 outputs in physical layout; residual partials
-  int32_t n_red_blocks, pub_mask;   // progress is published when (tau & pub_mask) == pub_mask
+  int32_t n_red_blocks, pub_mask;   // progress is published when (t & pub_mask) == pub_mask
   int32_t slack, fill_iso;          // fill_iso: (re)write the constant isothermal ghost planes (first iteration only)
   // ghost planes to fill in this iteration: (octant, axis) segments and their offsets in one flat index space
   int32_t gseg_n, gseg_oa[24];
@@ -127,11 +117,10 @@ template <typename T> struct alignas(16) Bte2Mom { T v[4]; };
 
 #define BTE2_HD __host__ __device__ __forceinline__
 
-// skewed cell index: oriented i', j' of the class, physical k.  One ROW = the 128 cells (k parity, jj, J) a warp
-// touches in one step (u = i' + J is the warp's local step): [k/2][ty][u][k&1][jj][J]
+// skewed cell index: oriented i', j' of the class, physical k
 BTE2_HD int64_t sk2_index(int nty, int NU, int ip, int jp, int k) {
   const int ty = jp >> 6, r = jp & 63, J = r >> 1, jj = r & 1;
-  return (((((int64_t)(k >> 1) * nty + ty) * NU + (ip + J)) * 2 + (k & 1)) * 2 + jj) * 32 + J;
+  return ((((int64_t)k * nty + ty) * NU + (ip + J)) * 2 + jj) * 32 + J;
 }
 // x planes: [tile][b][K][kk][jj][chunk][J], chunk = p / CP
 template <typename T>
@@ -139,17 +128,17 @@ BTE2_HD int64_t xpl2_index(const Bte2Dev &P, int ty, int tz, int b, int K, int k
   constexpr int NCH = BTE2_P * sizeof(T) / 16;
   return ((((((int64_t)(tz * P.nty + ty) * P.B + b) * P.W + K) * 2 + kk) * 2 + jj) * NCH + ch) * 32 + J;
 }
-// y planes: [slot][tz][g][K][i'][b in g][kk][chunk]: one row per (warp, step) and band group
+// y planes: [slot][tz][b][K][i'][kk][chunk]
 template <typename T>
 BTE2_HD int64_t ypl2_index(const Bte2Dev &P, int slot, int tz, int b, int K, int ip, int kk, int ch) {
-  constexpr int NCH = BTE2_P * sizeof(T) / 16, NBM = BTE2_NBMAX(T);
-  return (((((((int64_t)(slot * P.ntz + tz) * P.G + b / NBM) * P.W + K) * P.nx + ip) * NBM + b % NBM) * 2 + kk) * NCH + ch);
+  constexpr int NCH = BTE2_P * sizeof(T) / 16;
+  return (((((int64_t)(slot * P.ntz + tz) * P.B + b) * P.W + K) * P.nx + ip) * 2 + kk) * NCH + ch;
 }
-// z planes: [slot][ty][g][u][b in g][jj][chunk][J], u = i' + J: one row per step and band group
+// z planes: [slot][ty][b][u][jj][chunk][J], u = i' + J
 template <typename T>
 BTE2_HD int64_t zpl2_index(const Bte2Dev &P, int slot, int ty, int b, int u, int jj, int ch, int J) {
-  constexpr int NCH = BTE2_P * sizeof(T) / 16, NBM = BTE2_NBMAX(T);
-  return (((((((int64_t)(slot * P.nty + ty) * P.G + b / NBM) * P.NU + u) * NBM + b % NBM) * 2 + jj) * NCH + ch) * 32 + J);
+  constexpr int NCH = BTE2_P * sizeof(T) / 16;
+  return (((((int64_t)(slot * P.nty + ty) * P.B + b) * P.NU + u) * 2 + jj) * NCH + ch) * 32 + J;
 }
 
 #ifdef __CUDACC__
@@ -162,44 +151,27 @@ __device__ __forceinline__ int ld_acquire_gpu(const int *p) {
 __device__ __forceinline__ void st_release_gpu(int *p, int v) {
   asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
+template <int BYTES>
+__device__ __forceinline__ void cp_async(unsigned d, const void *gsrc) {   // d: shared-window address
+  if (BYTES == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+  else if (BYTES == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+  else if (BYTES == 4) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// split CTA barrier (BTE2_SPLITBAR): arrive once the step's shared-memory traffic is done, wait after the moment store
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-// mbarriers (shared memory)
 __device__ __forceinline__ void mbar_init(uint64_t *b, int count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
 }
-__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void mbar_arrive(uint64_t *b) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory"); }
-__device__ __forceinline__ void mbar_expect(uint64_t *b, unsigned bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
-}
-// The wait loop lives inside ONE asm statement (a C++ loop around try_wait is a divergent loop for the compiler).
 __device__ __forceinline__ void mbar_wait(uint64_t *b, unsigned parity) {
   asm volatile(
       "{\n.reg .pred P1;\nLAB_WAIT:\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n@P1 bra DONE;\nbra LAB_WAIT;\nDONE:\n}" ::"r"(smem_u32(b)),
       "r"(parity)
       : "memory");
 }
-// 1-D bulk copies (TMA).  Loads complete on an mbarrier; stores / reductions are tracked in bulk groups.
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src), "r"(bytes),
-               "r"(smem_u32(bar))
-               : "memory");
-}
-__device__ __forceinline__ void bulk_s2g(void *dst, const void *src, unsigned bytes) {
-  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
-}
-template <typename T> __device__ __forceinline__ void bulk_red_add(void *dst, const void *src, unsigned bytes);
-template <> __device__ __forceinline__ void bulk_red_add<float>(void *dst, const void *src, unsigned bytes) {
-  asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
-}
-template <> __device__ __forceinline__ void bulk_red_add<double>(void *dst, const void *src, unsigned bytes) {
-  asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f64 [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
-template <int N> __device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory"); }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
-__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 template <typename T> __device__ __forceinline__ Bte2Chunk<T> ldcg_chunk(const Bte2Chunk<T> *p) {
   const float4 v = __ldcg(reinterpret_cast<const float4 *>(p));
@@ -209,7 +181,7 @@ template <typename T> __device__ __forceinline__ Bte2Chunk<T> ldcg_chunk(const B
 }
 // packed pairs of directions: fp32 uses the sm_100 two-wide FMA (FFMA2: two FMAs per issue slot, which frees
 // issue slots for the non-FMA instructions of the step); fp64 is two scalar DFMAs.
-// Measured on B200 (bench/microbench_fma.cu): FFMA2 with two vector-register
+// Measured on B200 (csrc/microbench_fma_forms.cu, profiles/r01_fma_forms_microbench.txt): FFMA2 with two vector-register
 // operands and a uniform-register pair (the form used here) runs at the full FMA rate, 124.6 of 128 FMA/clk/SM.
 template <typename T> struct Bte2V2;
 template <> struct Bte2V2<float> { typedef float2 t; };
@@ -223,112 +195,154 @@ __device__ __forceinline__ void acc2(float2 &m, float2 w, float2 e) { m = __ffma
 __device__ __forceinline__ void acc2(double2 &m, double2 w, double2 e) { m.x = fma(w.x, e.x, m.x); m.x = fma(w.y, e.y, m.x); }
 __device__ __forceinline__ float2 mk2(float a, float b) { return make_float2(a, b); }
 __device__ __forceinline__ double2 mk2(double a, double b) { return make_double2(a, b); }
+template <typename T> __device__ __forceinline__ T shfl_up1(T v);
+template <> __device__ __forceinline__ float shfl_up1<float>(float v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+template <> __device__ __forceinline__ double shfl_up1<double>(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
 
-// shared-memory carve-up of one CTA.  D = prefetch distance in steps (ring of D+1 buffers).  Every [K] slice is
-// private to warp K except zex, which warp K writes and warp K+1 reads.
+// shared-memory carve-up of one CTA.  D = prefetch distance in steps (ring of D+1 buffers).
 template <typename T, int NB, int W, int D> struct Bte2Smem {
   static constexpr int CP = 16 / sizeof(T);            // directions per 16-byte chunk
   static constexpr int NCH = BTE2_P / CP;              // chunks per band
+  static constexpr int NC = NB * NCH;                  // chunks per row and step
   typedef Bte2Chunk<T> Ch;
-  Ch zex[2][W][NB][2][NCH][32];      // [parity][K][b][jj][chunk][lane]: kk=1 rows of warp K (= one z-plane row)
-  Ch zin0[D + 1][NB][2][NCH][32];    // [ring] z inflow row of warp 0
-  Ch ybuf[D + 1][W][NB][2][NCH];     // [ring][K][b][kk][chunk]: y inflow of lane 0 (= one y-plane row)
-  Ch yout[2][W][NB][2][NCH];         // [parity][K]: y outflow row (jj=1 rows of lane Jl), stored one step later
-  Ch ylast[W][NB][2][NCH];           // y outflow row of the last cell of the tile row
-  Bte2Mom<T> mst[W][2][2][32];       // [K][k parity][jj][lane]: the step's moment sums (= one accumulator row)
-  Bte2Pair<T> inp[D + 1][W][2][2][32];   // [ring][K][k parity][jj][lane] (dT, Q/sumC) (= one cell row)
-  uint32_t codes[D + 1][W][32];      // [ring][K][lane] cell bytes of the thread's patch (masked grids only)
-};
-// mbarriers of one CTA (same for every NB).  They are initialised once per kernel and never re-initialised: every warp
-// carries two step counters across its units, nf = steps it has run (uses of its full[] ring, and -- for K >= 1 -- of
-// zfull / zempty [.][K-1], because warp K-1 serves warp K exactly in the units where warp K runs) and nd = steps it has
-// run in units where warp K+1 runs too (uses of zfull / zempty [.][K]).  Slot = count % ring, phase parity = count / ring.
-template <int W> struct Bte2Bars {
-  uint64_t full[3][W];               // bulk loads of ring slot s of warp K have landed (tx count)
-  uint64_t zfull[2][W];              // warp K has written zex[slot][K]
-  uint64_t zempty[2][W];             // warp K+1 has read zex[slot][K]
+  Ch zex[2][W][2][NC][32];           // [parity][K][jj][chunk][lane]: kk=1 rows of warp K, read by warp K+1 / copied out
+  Ch zin0[D + 1][2][NC][32];         // staged z inflow plane of warp 0
+  Ch ybuf[D + 1][W][2][NC];          // [ring][warp][kk][chunk]: y inflow of lane 0
+  Ch yst[2][W][2 * NC];              // [parity][warp][kk*NC + chunk]: jj=1 rows of lane Jl, copied out one step later
+  Bte2Mom<T> mold[BTE2_MDIST(T) + 1][2][2][W * 32];  // [ring][kk][jj][tid] previous content of the moment accumulator
+  Bte2Pair<T> inp[D + 1][2][2][W * 32];    // [ring][kk][jj][tid] (dT, Q/sumC) of the cell
+  uint32_t codes[D + 1][W * 32];           // [ring][tid] cell bytes of the thread's patch (masked grids only)
 };
 
 // ------------------------------------------------------------------ one unit = (octant, band group, tile)
 template <typename T, int NB, int W, int D, bool MASKED>
 __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<T> &CF, const Bte2Unit &un,
-                                              unsigned char *smem_raw, Bte2Bars<W> *BR, int unit, unsigned &nf, unsigned &nd) {
+                                              unsigned char *smem_raw, int unit, uint64_t *stepbar, unsigned &bpar) {
   typedef Bte2Smem<T, NB, W, D> SM;
   SM *S = reinterpret_cast<SM *>(smem_raw);
-  constexpr int CP = SM::CP, NCH = SM::NCH, R = D + 1, NBM = BTE2_NBMAX(T);
+  constexpr int CP = SM::CP, NCH = SM::NCH, NC = SM::NC, NT = W * 32, R = D + 1;
+  // the accumulator rows of step t + 1 + MDIST are prefetched right after ensure(t + D) (split barrier): their publication
+  // upstream is only known if D >= 1 + MDIST
+  static_assert(D >= 1 + BTE2_MDIST(T), "prefetch distance too short for the accumulator prefetch");
   typedef Bte2Chunk<T> Ch;
   const unsigned FULL = 0xffffffffu;
-  const int J = threadIdx.x & 31, K = threadIdx.x >> 5;
+  const int tid = threadIdx.x, J = tid & 31, K = tid >> 5;
   const Bte2Oct &O = P.oct[un.oct];
-  const int ty = un.ty, tz = un.tz;
-  // first band of the unit = band group of this CTA = blockIdx.y: only such values stay on the uniform datapath in
-  // this kernel (and the coefficient addressing with them)
-  const int b0 = (int)blockIdx.y * NBM;
+  const int ty = un.ty, tz = un.tz, b0 = un.b0;
   const int jp0 = ty * 64 + 2 * J, kp0 = tz * 2 * W + 2 * K;
   // ny and nz are even on this path (host check): a patch is valid or invalid as a whole, and the last
   // valid row of a tile is always the jj = 1 / kk = 1 row of lane Jl / warp Kl
-  if (__all_sync(FULL, kp0 >= P.nz)) return;           // warp without rows (ragged last z tile, two-layer 2-D slabs)
-  const bool vthread = jp0 < P.ny;
+  const bool vthread = (jp0 < P.ny) && (kp0 < P.nz);
   const int Jl = (min(P.ny, (ty + 1) * 64) - 1 - ty * 64) >> 1, Kl = (min(P.nz, (tz + 1) * 2 * W) - 1 - tz * 2 * W) >> 1;
-  const int ulast = P.nx - 1 + Jl;                     // last local step with an active lane
   const bool first = un.dep_prev < 0;                  // first band group of this octant: M is written, not added to
   const int ebase = P.epoch << 16;
-  const int zf = O.sz < 0 ? 1 : 0;                     // oriented row kk is the physical k parity kk ^ zf
+  // shared-window address for cp.async (hoisting one base address out of the step loop measured slower in fp32)
+  auto saddr = [&](const void *ptr) { return (unsigned)__cvta_generic_to_shared(ptr); };
 
   const Ch *xin = reinterpret_cast<const Ch *>(O.xsrc);
   Ch *xout = reinterpret_cast<Ch *>(O.xdst);
+  Bte2Mom<T> *M = reinterpret_cast<Bte2Mom<T> *>(O.M);
+  const Bte2Pair<T> *dTQ = reinterpret_cast<const Bte2Pair<T> *>(P.dTQ[O.cls]);
 
-  // ---- global rows of this warp (lane 0 issues the copies); all advance by a constant stride per step
-  const int k2 = (O.sz > 0 ? kp0 : P.nz - 2 - kp0) >> 1;
-  const int64_t row0 = ((int64_t)k2 * P.nty + ty) * P.NU;                     // cell-row index of step 0
-  const Bte2Pair<T> *dTQrow = reinterpret_cast<const Bte2Pair<T> *>(P.dTQ[O.cls]) + row0 * 128;
-  Bte2Mom<T> *Mrow = reinterpret_cast<Bte2Mom<T> *>(O.M) + row0 * 128;
-  const uint32_t *cprow = MASKED ? P.codeP[O.cls] + row0 * 32 : nullptr;
-  constexpr int YROW = NBM * 2 * NCH, ZROW = NBM * 2 * NCH * 32;              // chunks per plane row
-  constexpr unsigned ROWB = 128u * (unsigned)sizeof(Bte2Pair<T>), MB = 128u * (unsigned)sizeof(Bte2Mom<T>);
-  constexpr unsigned YB = NB * 2u * NCH * 16u, ZB = NB * 2u * NCH * 32u * 16u;
-  const Ch *ysrc = (ty == 0 ? reinterpret_cast<const Ch *>(O.ysrc0) : reinterpret_cast<const Ch *>(O.ypl) + ypl2_index<T>(P, ty, 0, 0, 0, 0, 0, 0)) +
-                   ypl2_index<T>(P, 0, tz, b0, K, 0, 0, 0);
-  Ch *ydst = (ty == P.nty - 1 ? reinterpret_cast<Ch *>(O.ydstN) : reinterpret_cast<Ch *>(O.ypl) + ypl2_index<T>(P, ty + 1, 0, 0, 0, 0, 0, 0)) +
-             ypl2_index<T>(P, 0, tz, b0, K, 0, 0, 0);
+  // cell index of row (jj,kk) at step t: cbase[kk] + jj*32 + (t - K) * 64
+  int64_t cbase[2];
+#pragma unroll
+  for (int kk = 0; kk < 2; ++kk) {
+    const int kp = kp0 + kk, k = vthread ? (O.sz > 0 ? kp : P.nz - 1 - kp) : 0;
+    cbase[kk] = (((int64_t)k * P.nty + ty) * P.NU) * 64 + J - (int64_t)K * 64;
+  }
+  // voxel mask: patch-code stream of this thread, face indices of this octant
+  const int fu[3] = {O.sx > 0 ? 0 : 1, O.sy > 0 ? 2 : 3, O.sz > 0 ? 4 : 5};      // upwind faces x, y, z
+  const uint32_t *cpsrc = nullptr;
+  if (MASKED) {
+    const int kz = (vthread ? (O.sz > 0 ? kp0 : P.nz - 2 - kp0) : 0) >> 1;
+    cpsrc = P.codeP[O.cls] + (((int64_t)kz * P.nty + ty) * P.NU) * 32 + J - (int64_t)K * 32;
+  }
+  // plane pointers of this thread at step 0; all advance by a constant stride per step
+  //   z inflow staging: element e = tid + q*NT of the [b][jj][ch][lane] block of step u
   const Ch *zsrc = (tz == 0 ? reinterpret_cast<const Ch *>(O.zsrc0) : reinterpret_cast<const Ch *>(O.zpl) + zpl2_index<T>(P, tz, 0, 0, 0, 0, 0, 0)) +
                    zpl2_index<T>(P, 0, ty, b0, 0, 0, 0, 0);
+  const int64_t zstep = 2 * NCH * 32, zband = (int64_t)P.NU * 2 * NCH * 32;
   Ch *zdst = (tz == P.ntz - 1 ? reinterpret_cast<Ch *>(O.zdstN) : reinterpret_cast<Ch *>(O.zpl) + zpl2_index<T>(P, tz + 1, 0, 0, 0, 0, 0, 0)) +
              zpl2_index<T>(P, 0, ty, b0, 0, 0, 0, 0);
+  //   y planes: lane l < 2*NC of warp K loads chunk (b, kk, ch) of the cell i' = t - K
+  const int yb = J / (2 * NCH), ykk = (J / NCH) & 1, ych = J % NCH;
+  const Ch *ysrc = (ty == 0 ? reinterpret_cast<const Ch *>(O.ysrc0) : reinterpret_cast<const Ch *>(O.ypl) + ypl2_index<T>(P, ty, 0, 0, 0, 0, 0, 0)) +
+                   ypl2_index<T>(P, 0, tz, b0 + (J < 2 * NC ? yb : 0), K, 0, ykk, ych) - (int64_t)K * 2 * NCH;
+  Ch *ydst = (ty == P.nty - 1 ? reinterpret_cast<Ch *>(O.ydstN) : reinterpret_cast<Ch *>(O.ypl) + ypl2_index<T>(P, ty + 1, 0, 0, 0, 0, 0, 0)) +
+             ypl2_index<T>(P, 0, tz, b0 + (J < 2 * NC ? yb : 0), K, 0, ykk, ych);
 
-  // ---- progress of the warps this one follows: lanes 0..2 keep the last value seen in a register.
-  //   lane 0: warp K of the upstream tile in y   (its y outflow row of cell i' is complete once it published i' + 33)
-  //   lane 1: last warp of the upstream tile in z (warp 0 only; z outflow row u complete once it published u + 1)
-  //   lane 2: warp K of the previous band group on this tile (its addition to accumulator row u: published u + 1)
-  const int mydep = J == 0 ? (un.dep_y >= 0 ? un.dep_y * W + K : -1)
-                  : (J == 1 ? ((K == 0 && un.dep_z >= 0) ? un.dep_z * W + (W - 1) : -1)
-                  : (J == 2 ? (un.dep_prev >= 0 ? un.dep_prev * W + K : -1) : -1));
-  const int mylag = J == 0 ? BTE2_YLAG : 1;
-  const int mycap = J == 0 ? P.nx - 1 : ulast;         // last step that reads from the dependency
+  // ---- progress of the units this one follows: lanes 0..2 of warp 0 keep the last value seen in a register
+  const int mydep = tid == 0 ? un.dep_y : (tid == 1 ? un.dep_z : (tid == 2 ? un.dep_prev : -1));
+  const int mylag = tid == 0 ? 33 : (tid == 1 ? W + 1 : 1);
   int seen = 0, peek = 0;
-  bool sawnew = false;
-  auto ensure = [&](int t1) {          // everything step t1 takes from the other unit has been published
-    if (mydep >= 0) {
-      const int need = min(t1, mycap) + mylag;
-      if (peek - ebase > seen) { seen = peek - ebase; sawnew = true; }
-      if (seen < need) {
+  auto ensure = [&](int t1) {          // everything step t1 reads from other units has been published
+    if (mydep >= 0 && !BTE2_DBGBIT(P, 4)) {
+      seen = max(seen, peek - ebase);
+      if (seen < t1 + mylag) {
         int v;
-        while ((v = ld_acquire_gpu(P.prog + mydep) - ebase) < need) __nanosleep(64);
-        seen = v; sawnew = true;
+        while ((v = ld_acquire_gpu(P.prog + mydep) - ebase) < t1 + mylag) __nanosleep(64);
+        seen = v;
       }
     }
   };
 
-  // ---- bulk loads of everything step t1 consumes into ring slot sl (lane 0)
-  auto issue = [&](int t1, int sl) {
-    if (t1 > ulast) return;
-    uint64_t *bar = &BR->full[sl][K];
-    const bool yok = t1 < P.nx, zok = K == 0;
-    mbar_expect(bar, ROWB + (MASKED ? 128u : 0u) + (yok ? YB : 0u) + (zok ? ZB : 0u));
-    bulk_g2s(&S->inp[sl][K][0][0][0], dTQrow + (int64_t)t1 * 128, ROWB, bar);
-    if (MASKED) bulk_g2s(&S->codes[sl][K][0], cprow + (int64_t)t1 * 32, 128u, bar);
-    if (yok) bulk_g2s(&S->ybuf[sl][K][0][0][0], ysrc + (int64_t)t1 * YROW, YB, bar);
-    if (zok) bulk_g2s(&S->zin0[sl][0][0][0][0], zsrc + (int64_t)t1 * ZROW, ZB, bar);
+  // ---- previous content of the moment accumulator for step t1 (own commit group, one step ahead)
+  auto prefetch_m = [&](int t1) {
+    const int ip1 = t1 - J - K;
+    if (!first && !BTE2_DBGBIT(P, 2) && vthread && ip1 >= 0 && ip1 < P.nx) {
+#pragma unroll
+      for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+        for (int jj = 0; jj < 2; ++jj) {
+          const int64_t ci = cbase[kk] + jj * 32 + (int64_t)t1 * 64;
+#pragma unroll
+          for (int h = 0; h < (int)sizeof(Bte2Mom<T>) / 16; ++h)
+            cp_async<16>(saddr(&S->mold[t1 % (BTE2_MDIST(T) + 1)][kk][jj][tid]) + 16 * h, reinterpret_cast<const char *>(M + ci) + 16 * h);
+        }
+    }
+  };
+  // ---- outflow faces of step t1 (staged in shared memory by the step) -> global planes, coalesced
+  auto copy_out = [&](int t1) {
+    const int par = (t1 & 1) ^ 1;                      // buffer the step wrote
+    if (!BTE2_DBGBIT(P, 1) && kp0 < P.nz) {
+      const int ipl = t1 - Jl - K;                     // cell lane Jl of this warp finished in step t1
+      if (J < 2 * NC && ipl >= 0 && ipl < P.nx) ydst[(int64_t)ipl * 2 * NCH] = S->yst[par][K][ykk * NC + yb * NCH + ych];
+    }
+    const int ul = t1 - Kl;
+    if (!BTE2_DBGBIT(P, 1) && ul >= 0 && ul < P.NU) {
+#pragma unroll
+      for (int q = 0; q < (2 * NC * 32) / NT; ++q) {
+        const int e = tid + q * NT, b = e / (2 * NCH * 32), rem = e % (2 * NCH * 32);
+        zdst[b * zband + ul * zstep + rem] = (&S->zex[par][Kl][0][b * NCH][0])[(rem / (NCH * 32)) * (NC * 32) + (rem % (NCH * 32))];
+      }
+    }
+  };
+  // ---- asynchronous prefetch (global -> shared) of everything step t1 consumes
+  auto prefetch = [&](int t1, int rb) {                // rb = t1 % R, the ring slot of step t1
+    const int ip1 = t1 - J - K;
+    if (vthread && ip1 >= 0 && ip1 < P.nx) {
+#pragma unroll
+      for (int kk = 0; kk < 2; ++kk) {
+#pragma unroll
+          for (int jj = 0; jj < 2; ++jj) {
+            const int64_t ci = cbase[kk] + jj * 32 + (int64_t)t1 * 64;
+            cp_async<sizeof(Bte2Pair<T>)>(saddr(&S->inp[rb][kk][jj][tid]), dTQ + ci);
+          }
+        }
+    }
+    if (MASKED && vthread && ip1 >= 0 && ip1 < P.nx) cp_async<4>(saddr(&S->codes[rb][tid]), cpsrc + (int64_t)t1 * 32);
+    if (t1 < P.NU && !BTE2_DBGBIT(P, 8)) {
+#pragma unroll
+      for (int q = 0; q < (2 * NC * 32) / NT; ++q) {
+        const int e = tid + q * NT, b = e / (2 * NCH * 32), rem = e % (2 * NCH * 32);
+        cp_async<16>(saddr(&S->zin0[rb][0][b * NCH][0] + (rem / (NCH * 32)) * (NC * 32) + (rem % (NCH * 32))), zsrc + b * zband + t1 * zstep + rem);
+      }
+    }
+    {
+      const int ipy = t1 - K;
+      if (J < 2 * NC && ipy >= 0 && ipy < P.nx) cp_async<16>(saddr(&S->ybuf[rb][K][ykk][yb * NCH + ych]), ysrc + (int64_t)t1 * 2 * NCH);
+    }
   };
 
   // ---- x inflow -> carry registers (kept untouched by a thread until its first active step)
@@ -347,48 +361,45 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
           for (int q = 0; q < CP; q += 2) c[jj][kk][(b * BTE2_P + ch * CP + q) / 2] = mk2(v.v[q], v.v[q + 1]);
         }
 
-  // ---- prologue: dependencies of the first D steps (loads) and of step 0 (accumulator), first loads
-  if (J < 2) ensure(D + P.slack); else if (J == 2) ensure(0);
-  __syncwarp();
-  if (J == 0) {
-    fence_proxy_async();                               // what the acquires made visible was written through the async proxy
+  ensure(D + P.slack);
+  __syncthreads();
 #pragma unroll
-    for (int t1 = 0; t1 < D; ++t1) issue(t1, (int)((nf + t1) % R));
+  for (int t1 = 0; t1 < D; ++t1) {
+    if (t1 == 0 && BTE2_MDIST(T) == 1) prefetch_m(0);
+    prefetch(t1, t1); cp_async_commit();
   }
-  sawnew = false;
+#if BTE2_SPLITBAR
+  prefetch_m(BTE2_MDIST(T)); cp_async_commit();        // steady state: issued in the barrier window of the previous step
+#endif
+  cp_async_wait<D - 1>();
+  __syncthreads();
 
   T bcx[NB], bcy[NB];
 #pragma unroll
   for (int b = 0; b < NB; ++b) { bcx[b] = CF.bc[b0 + b][0]; bcy[b] = CF.bc[b0 + b][1]; }
-  const int srcl = J == 0 ? Jl : J - 1;                // y exchange: rotate by one lane; lane 0 receives the tile's y outflow
 
   // one (band, chunk) of the 2x2 patch: FAST = every lane of the warp is active (no predication)
   auto chunk = [&](auto fastc, int b, int ch, const V2 (&r)[2][2], V2 (&m)[2][2][4], int rb, int cur, bool act,
                    const Ch *__restrict__ zrd, Ch *__restrict__ zwr) {
     constexpr bool FAST = decltype(fastc)::value;
     constexpr int NP = CP / 2;                         // direction pairs per chunk
-    const int h0 = (b * BTE2_P + ch * CP) / 2, zo = b * 2 * NCH + ch;   // zo: [b][jj = 0][ch] of a z row
-    // y inflow: lane J-1's jj=1 rows of the previous step; lane 0 receives lane Jl's (the tile's y outflow, which it
-    // stages for the bulk store) and takes its own inflow from the staged plane row
+    const int h0 = (b * BTE2_P + ch * CP) / 2, cn = b * NCH + ch;
+    // y inflow: lane J-1's jj=1 rows of the previous step; lane 0: the staged plane
     V2 yin[2][NP];
 #pragma unroll
     for (int kk = 0; kk < 2; ++kk)
 #pragma unroll
-      for (int q = 0; q < NP; ++q) yin[kk][q] = mk2(__shfl_sync(FULL, c[1][kk][h0 + q].x, srcl), __shfl_sync(FULL, c[1][kk][h0 + q].y, srcl));
+      for (int q = 0; q < NP; ++q) yin[kk][q] = mk2(shfl_up1<T>(c[1][kk][h0 + q].x), shfl_up1<T>(c[1][kk][h0 + q].y));
     if (J == 0) {
 #pragma unroll
       for (int kk = 0; kk < 2; ++kk) {
-        Ch o;
-#pragma unroll
-        for (int q = 0; q < NP; ++q) { o.v[2 * q] = yin[kk][q].x; o.v[2 * q + 1] = yin[kk][q].y; }
-        S->yout[cur][K][b][kk][ch] = o;
-        const Ch v = S->ybuf[rb][K][b][kk][ch];
+        const Ch v = S->ybuf[rb][K][kk][cn];
 #pragma unroll
         for (int q = 0; q < NP; ++q) yin[kk][q] = mk2(v.v[2 * q], v.v[2 * q + 1]);
       }
     }
-    // z inflow: warp K-1's kk=1 rows of the same step, or the staged plane row for warp 0
-    const Ch z0 = zrd[zo * 32], z1 = zrd[(zo + NCH) * 32];
+    // z inflow: warp K-1's kk=1 rows of the previous step, or the staged plane for warp 0
+    const Ch z0 = zrd[cn * 32], z1 = zrd[(NC + cn) * 32];
     if (FAST || act) {
       Ch o0, o1;
 #pragma unroll
@@ -411,36 +422,31 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
         acc2(m[0][1][0], w0, e01); acc2(m[0][1][1], w1, e01); acc2(m[0][1][2], w2, e01); acc2(m[0][1][3], w3, e01);
         acc2(m[1][1][0], w0, e11); acc2(m[1][1][1], w1, e11); acc2(m[1][1][2], w2, e11); acc2(m[1][1][3], w3, e11);
       }
-      zwr[zo * 32] = o0; zwr[(zo + NCH) * 32] = o1;
+      zwr[cn * 32] = o0; zwr[(NC + cn) * 32] = o1;
     }
   };
 
   // the same (band, chunk) on a patch that contains void cells or solid/void interface faces: every cell
   // takes its upwind values through selects (interface inflow g instead of the neighbour) and void cells hold 0.
   // cb[c] = code byte, g[c][axis] = interface inflow of cell c = A (0,0), B (1,0), C (0,1), D (1,1).
-  const int fu[3] = {O.sx > 0 ? 0 : 1, O.sy > 0 ? 2 : 3, O.sz > 0 ? 4 : 5};      // upwind faces x, y, z
-  auto chunk_masked = [&](int b, int ch, const V2 (&r)[2][2], V2 (&m)[2][2][4], int rb, int cur, bool act, const uint32_t (&cb)[4],
+  auto chunk_masked = [&](int b, int ch, const V2 (&r)[2][2], V2 (&m)[2][2][4], int rb, bool act, const uint32_t (&cb)[4],
                           const T (&g)[4][3], const Ch *__restrict__ zrd, Ch *__restrict__ zwr) {
     constexpr int NP = CP / 2;
-    const int h0 = (b * BTE2_P + ch * CP) / 2, zo = b * 2 * NCH + ch;
+    const int h0 = (b * BTE2_P + ch * CP) / 2, cn = b * NCH + ch;
     V2 yin[2][NP];
 #pragma unroll
     for (int kk = 0; kk < 2; ++kk)
 #pragma unroll
-      for (int q = 0; q < NP; ++q) yin[kk][q] = mk2(__shfl_sync(FULL, c[1][kk][h0 + q].x, srcl), __shfl_sync(FULL, c[1][kk][h0 + q].y, srcl));
+      for (int q = 0; q < NP; ++q) yin[kk][q] = mk2(shfl_up1<T>(c[1][kk][h0 + q].x), shfl_up1<T>(c[1][kk][h0 + q].y));
     if (J == 0) {
 #pragma unroll
       for (int kk = 0; kk < 2; ++kk) {
-        Ch o;
-#pragma unroll
-        for (int q = 0; q < NP; ++q) { o.v[2 * q] = yin[kk][q].x; o.v[2 * q + 1] = yin[kk][q].y; }
-        S->yout[cur][K][b][kk][ch] = o;
-        const Ch v = S->ybuf[rb][K][b][kk][ch];
+        const Ch v = S->ybuf[rb][K][kk][cn];
 #pragma unroll
         for (int q = 0; q < NP; ++q) yin[kk][q] = mk2(v.v[2 * q], v.v[2 * q + 1]);
       }
     }
-    const Ch z0 = zrd[zo * 32], z1 = zrd[(zo + NCH) * 32];
+    const Ch z0 = zrd[cn * 32], z1 = zrd[(NC + cn) * 32];
     if (!act) return;                                  // (shuffles above stay warp-convergent)
     auto up = [&](uint32_t code, int axis, T gv, V2 v) { return (code >> (1 + fu[axis])) & 1u ? mk2(gv, gv) : v; };
     auto keep = [&](uint32_t code, V2 v) { return (code & 1u) ? v : mk2((T)0, (T)0); };
@@ -469,20 +475,22 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
       acc2(m[0][1][0], w0, e01); acc2(m[0][1][1], w1, e01); acc2(m[0][1][2], w2, e01); acc2(m[0][1][3], w3, e01);
       acc2(m[1][1][0], w0, e11); acc2(m[1][1][1], w1, e11); acc2(m[1][1][2], w2, e11); acc2(m[1][1][3], w3, e11);
     }
-    zwr[zo * 32] = o0; zwr[(zo + NCH) * 32] = o1;
+    zwr[cn * 32] = o0; zwr[(NC + cn) * 32] = o1;
   };
 
-  const bool feeds = K < Kl;                           // warp K+1 runs in this unit and reads this warp's kk = 1 rows
-  int rb = (int)(nf % R), rbp = (rb + R - 1) % R;      // ring slots of step tau and of step tau - 1 (= step tau + D)
-  unsigned fph = (nf / R) & 1u;                        // phase parity of full[rb]
-  for (int tau = 0; tau <= ulast; ++tau) {
-    const int cur = tau & 1;                           // staging parity (y outflow row; z outflow row of the last warp)
-    const int zin = (int)(nf & 1u), zout = feeds ? (int)(nd & 1u) : cur;   // zex slots read (warp K-1's) / written
-    const int ip = tau - J;
+  int rb = 0, rbp = R - 1;                             // ring slots of step t and of step t - 1 (= step t + D)
+  for (int t = 0; t < P.nsteps; ++t) {
+    const int cur = t & 1;
+    const int ip = t - J - K;
     const bool act = vthread && ip >= 0 && ip < P.nx;
-    if (J == 0) issue(tau + D, rbp);
-    // progress of the units this one follows, for the END of this step (the load is in flight during the arithmetic)
-    if (J < 3 && mydep >= 0 && seen < min(tau + 1 + (J < 2 ? D : 0), mycap) + mylag) peek = ld_acquire_gpu(P.prog + mydep);
+#if !BTE2_SPLITBAR
+    prefetch_m(t + BTE2_MDIST(T));
+    cp_async_commit();
+#endif
+    prefetch(t + D, rbp);
+    cp_async_commit();
+    if (t > 0) copy_out(t - 1);
+    if (tid < 3 && mydep >= 0 && seen < t + 1 + D + mylag) peek = ld_acquire_gpu(P.prog + mydep);   // consumed by ensure() below
 
     V2 m[2][2][4];                                     // moment partial sums of even / odd directions
 #pragma unroll
@@ -492,18 +500,17 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
 #pragma unroll
         for (int q = 0; q < 4; ++q) m[a][b][q] = mk2((T)0, (T)0);
 
-    mbar_wait(&BR->full[rb][K], fph);                  // the rows of this step have landed
     Bte2Pair<T> in[2][2];
 #pragma unroll
     for (int kk = 0; kk < 2; ++kk)
 #pragma unroll
-      for (int jj = 0; jj < 2; ++jj) in[jj][kk] = S->inp[rb][K][kk ^ zf][jj][J];
+      for (int jj = 0; jj < 2; ++jj) in[jj][kk] = S->inp[rb][kk][jj][tid];
 
     // masked grids: code bytes of the patch, oriented cell (jj,kk) -> byte (physical parities)
     uint32_t cb[4] = {1u, 1u, 1u, 1u};
     bool plain = true, live = act;                     // live: the patch holds at least one solid cell
     if (MASKED) {
-      const uint32_t code = act ? S->codes[rb][K][J] : 0x01010101u;
+      const uint32_t code = act ? S->codes[rb][tid] : 0x01010101u;
       plain = code == 0x01010101u;
       live = act && (code & 0x01010101u) != 0;
 #pragma unroll
@@ -514,13 +521,11 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     }
     const bool fast = __all_sync(FULL, act && plain);
     const bool slowmask = MASKED && __any_sync(FULL, live && !plain);
-    const Ch *__restrict__ zrd = K == 0 ? &S->zin0[rb][0][0][0][J] : &S->zex[zin][K - 1][0][0][0][J];
-    Ch *__restrict__ zwr = &S->zex[zout][K][0][0][0][J];
-    // neighbour-only synchronisation: warp K-1 has written its rows of this step; warp K+1 has read the buffer
-    // this step overwrites (written two of its uses ago)
-    if (K > 0) mbar_wait(&BR->zfull[zin][K - 1], (nf >> 1) & 1u);
-    if (feeds && nd >= 2u) mbar_wait(&BR->zempty[zout][K], ((nd >> 1) & 1u) ^ 1u);
-
+    const Ch *__restrict__ zrd = K == 0 ? &S->zin0[rb][0][0][J] : &S->zex[cur][K - 1][0][0][J];
+    Ch *__restrict__ zwr = &S->zex[cur ^ 1][K][0][0][J];
+    // warps without a valid row (ragged last z tile; 3 of 4 warps of a two-layer 2-D slab) and warps that are
+    // entirely before their first or after their last cell skip the arithmetic (they still stage and synchronise)
+    if (__any_sync(FULL, act))
 #pragma unroll
     for (int b = 0; b < NB; ++b) {
       V2 r[2][2];
@@ -545,19 +550,19 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
           for (int a = 0; a < 3; ++a) {
             g[cc][a] = (T)0;
             if (live && (cb[cc] & 1u) && ((cb[cc] >> (1 + fu[a])) & 1u))
-              g[cc][a] = P.iface_type == 0 ? (T)P.iface_e0[b0 + b]
+              g[cc][a] = (P.iface_type == 0 || BTE2_DBGBIT(P, 64)) ? (T)P.iface_e0[b0 + b]
                                            : reinterpret_cast<const T *>(P.Gi)[(int64_t)__ldg(P.iface + (int64_t)fu[a] * P.ncell + cph[cc]) * P.B + b0 + b];
           }
         }
 #pragma unroll
-        for (int ch = 0; ch < NCH; ++ch) chunk_masked(b, ch, r, m, rb, cur, live, cb, g, zrd, zwr);
+        for (int ch = 0; ch < NCH; ++ch) chunk_masked(b, ch, r, m, rb, live, cb, g, zrd, zwr);
         {
           // outgoing hemispherical partial sums at solid/void faces (diffuse interface, Eq. 6)
           uint32_t anydn = 0;
 #pragma unroll
           for (int cc = 0; cc < 4; ++cc)
             if (cb[cc] & 1u) anydn |= cb[cc] & ((2u << (fu[0] ^ 1)) | (2u << (fu[1] ^ 1)) | (2u << (fu[2] ^ 1)));
-          if (P.iface_type == 1 && live && anydn != 0) {
+          if (P.iface_type == 1 && live && anydn != 0 && !BTE2_DBGBIT(P, 128)) {
 #pragma unroll
             for (int cc = 0; cc < 4; ++cc) {
               const int jj = cc & 1, kk = cc >> 1;
@@ -592,68 +597,72 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
       }
     }
 
-    // the last cell of the tile row: lane Jl's jj = 1 rows are final (no later step rotates them out)
-    if (tau == ulast && J == Jl) {
+    if (BTE2_MDIST(T) == 0) cp_async_wait<D - 1>();   // the accumulator content fetched in THIS step has landed
+#if BTE2_SPLITBAR
+    cp_async_wait<D - 1>();            // everything step t+1 reads has landed
+    if (tid < 3) ensure(t + 1 + D);    // ... and what step t+1 prefetches has been published upstream
+    mbar_arrive(stepbar);              // this thread's shared-memory reads and writes of step t are done
+#endif
+    if (act) {
+      // (b) moments of this band group into the octant accumulator (one owner per cell and group)
 #pragma unroll
-      for (int b = 0; b < NB; ++b)
+      for (int kk = 0; kk < 2; ++kk)
+        if (!BTE2_DBGBIT(P, 2)) {
 #pragma unroll
-        for (int kk = 0; kk < 2; ++kk)
+          for (int jj = 0; jj < 2; ++jj) {
+            if (MASKED && !(cb[jj + 2 * kk] & 1u)) continue;      // void cell
+            Bte2Mom<T> o;
+            if (first) {
 #pragma unroll
-          for (int ch = 0; ch < NCH; ++ch) {
-            Ch o;
+              for (int q = 0; q < 4; ++q) o.v[q] = m[jj][kk][q].x + m[jj][kk][q].y;
+            } else {
+              const Bte2Mom<T> old = S->mold[t % (BTE2_MDIST(T) + 1)][kk][jj][tid];
 #pragma unroll
-            for (int q = 0; q < CP; q += 2) {
-              const V2 v = c[1][kk][(b * BTE2_P + ch * CP + q) / 2];
-              o.v[q] = v.x; o.v[q + 1] = v.y;
+              for (int q = 0; q < 4; ++q) o.v[q] = old.v[q] + (m[jj][kk][q].x + m[jj][kk][q].y);
             }
-            S->ylast[K][b][kk][ch] = o;
+            M[cbase[kk] + jj * 32 + (int64_t)t * 64] = o;
           }
-    }
-    if (J == 0) bulk_wait_read<0>();                   // the stores of the previous step have read their staging rows
-    __syncwarp();                                      // this warp's shared-memory reads and writes of the step are done
-    if (J == 0) {
-      if (feeds) mbar_arrive(&BR->zfull[zout][K]);
-      if (K > 0) mbar_arrive(&BR->zempty[zin][K - 1]);
-    }
-    // (b) moments of this band group -> staging row (zeros for cells this step does not own)
+        }
+      // y outflow rows (jj = 1 of lane Jl) -> staging buffer; written to the plane by copy_out() next step
+      if (J == Jl) {
 #pragma unroll
-    for (int kk = 0; kk < 2; ++kk)
+        for (int b = 0; b < NB; ++b)
 #pragma unroll
-      for (int jj = 0; jj < 2; ++jj) {
-        Bte2Mom<T> o;
-        const bool own = act && (!MASKED || (cb[jj + 2 * kk] & 1u));
+          for (int kk = 0; kk < 2; ++kk)
 #pragma unroll
-        for (int q = 0; q < 4; ++q) o.v[q] = own ? m[jj][kk][q].x + m[jj][kk][q].y : (T)0;
-        S->mst[K][kk ^ zf][jj][J] = o;
+            for (int ch = 0; ch < NCH; ++ch) {
+              Ch o;
+#pragma unroll
+              for (int q = 0; q < CP; q += 2) {
+                const V2 v = c[1][kk][(b * BTE2_P + ch * CP + q) / 2];
+                o.v[q] = v.x; o.v[q + 1] = v.y;
+              }
+              S->yst[cur ^ 1][K][kk * NC + b * NCH + ch] = o;
+            }
       }
-    fence_proxy_async_smem();                          // staging rows and zex (generic proxy) -> bulk stores (async proxy)
-    if (J < 3) ensure(tau + 1 + (J < 2 ? D : 0));      // what the next step issues (loads / accumulator addition)
-    if (sawnew) fence_proxy_async();                   // rows published through the async proxy -> this warp's bulk loads
-    const bool anynew = __any_sync(FULL, sawnew);      // (also orders the staging writes before lane 0's stores)
-    sawnew = false;
-    if (J == 0) {
-      if (anynew) fence_proxy_async();
-      // moments: the first band group of the octant writes the accumulator row, the others add to it in the L2
-      if (first) bulk_s2g(Mrow + (int64_t)tau * 128, &S->mst[K][0][0][0], MB);
-      else bulk_red_add<T>(Mrow + (int64_t)tau * 128, &S->mst[K][0][0][0], MB);
-      const int iy = tau - 1 - Jl;                     // y outflow row staged in this step (lane Jl's previous step)
-      if (iy >= 0) bulk_s2g(ydst + (int64_t)iy * YROW, &S->yout[cur][K][0][0][0], YB);
-      if (tau == ulast) bulk_s2g(ydst + (int64_t)(P.nx - 1) * YROW, &S->ylast[K][0][0][0], YB);
-      if (K == Kl) bulk_s2g(zdst + (int64_t)tau * ZROW, &S->zex[zout][K][0][0][0][0], ZB);
-      bulk_commit();
-      if ((tau & P.pub_mask) == P.pub_mask) {          // steps < tau are complete in global memory
-        bulk_wait<1>();
-        fence_proxy_async();
-        st_release_gpu(P.prog + unit * W + K, ebase + tau);
-      }
+    }
+#if BTE2_SPLITBAR
+    // accumulator rows of the step after next: their publication upstream is known since the previous barrier
+    // (ensure(t + D) covers step t + 1 + MDIST because D >= 1 + MDIST), and the ring slot was read just above
+    prefetch_m(t + 1 + BTE2_MDIST(T));
+    cp_async_commit();
+    mbar_wait(stepbar, bpar);          // every thread has arrived: the moment store above overlapped the wait
+    bpar ^= 1u;
+    __syncwarp();                      // yst rows written after the arrive are read by this warp's copy_out next step
+#else
+    cp_async_wait<D - 1>();            // everything step t+1 reads has landed
+    if (tid < 3) ensure(t + 1 + D);    // ... and what step t+1 prefetches has been published upstream
+    __syncthreads();
+#endif
+    if ((t & P.pub_mask) == P.pub_mask && tid == 0) {   // faces and moments of steps < t are in global memory
+      __threadfence();
+      st_release_gpu(P.prog + unit, ebase + t);
     }
     rbp = rb;
     rb = rb + 1 == R ? 0 : rb + 1;
-    if (rb == 0) fph ^= 1u;
-    nf += 1u;
-    nd += feeds ? 1u : 0u;
   }
-  if (J == 0) bulk_wait<0>();
+  cp_async_wait<0>();
+  copy_out(P.nsteps - 1);
 
   // ---- x outflow (carries are final: a thread stops updating them after its last active step)
 #pragma unroll
@@ -673,48 +682,29 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
           xout[xpl2_index<T>(P, ty, tz, b0 + b, K, kk, jj, ch, J)] = o;
         }
   __threadfence();
-  __syncwarp();
-  if (J == 0) {
-    fence_proxy_async();
-    st_release_gpu(P.prog + unit * W + K, ebase + 0xffff);
-  }
-}
-
-template <typename T, int NB, int W, bool MASKED>
-__device__ __forceinline__ void bte2_run_group(const Bte2Dev &P, const Bte2Coefs<T> &CF, unsigned char *smem_raw,
-                                               Bte2Bars<W> *bars, int *s_unit) {
-  constexpr int D = BTE2_DIST(W, T);
-  const int g = blockIdx.y;
-  unsigned nf = 0, nd = 0;                             // this warp's barrier use counters (see Bte2Bars)
-  for (;;) {
-    __syncthreads();                                   // every warp is done with the previous unit (shared memory is free)
-    if (threadIdx.x == 0) {
-      // groups get CTAs in proportion to their work: CTA (x, y) with x >= cta_count[y] leaves without taking a ticket
-      const int tk = (int)blockIdx.x < P.cta_count[g] ? P.gfirst[g] + atomicAdd(P.ticket + g, 1) : P.gfirst[g + 1];
-      *s_unit = tk < P.gfirst[g + 1] ? P.gorder[tk] : -1;
-    }
-    __syncthreads();
-    const int unit = *s_unit;
-    if (unit < 0) break;
-    const Bte2Unit un = P.units[unit];
-    bte2_run_unit<T, NB, W, D, MASKED>(P, CF, un, smem_raw, bars, unit, nf, nd);
-  }
+  __syncthreads();
+  if (tid == 0) st_release_gpu(P.prog + unit, ebase + 0xffff);
 }
 
 template <typename T, int W, bool MASKED>
 __global__ void __launch_bounds__(W * 32) bte2_sweep_kernel(const __grid_constant__ Bte2Dev P,
                                                             const __grid_constant__ Bte2Coefs<T> CF) {
-  extern __shared__ __align__(128) unsigned char bte2_smem_raw[];
-  constexpr int NBMAX = BTE2_NBMAX(T);
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int NBMAX = sizeof(T) == 4 ? 2 : 1, D = BTE2_DIST(W, T);
   __shared__ int s_unit;
-  __shared__ Bte2Bars<W> s_bars;
-  if (threadIdx.x == 0) {
-    uint64_t *b = reinterpret_cast<uint64_t *>(&s_bars);
-    for (int i = 0; i < (int)(sizeof(s_bars) / 8); ++i) mbar_init(b + i, 1);
-    fence_mbar_init();
+  __shared__ uint64_t s_stepbar;
+  unsigned bpar = 0;
+  if (BTE2_SPLITBAR && threadIdx.x == 0) mbar_init(&s_stepbar, W * 32);
+  for (;;) {
+    __syncthreads();
+    if (threadIdx.x == 0) s_unit = atomicAdd(P.ticket, 1);
+    __syncthreads();
+    const int unit = s_unit;
+    if (unit >= P.n_units) break;
+    const Bte2Unit un = P.units[unit];
+    if (NBMAX == 2 && un.nb == 2) bte2_run_unit<T, NBMAX, W, D, MASKED>(P, CF, un, smem_raw, unit, &s_stepbar, bpar);
+    else bte2_run_unit<T, 1, W, D, MASKED>(P, CF, un, smem_raw, unit, &s_stepbar, bpar);
   }
-  if (NBMAX == 2 && P.B - (int)blockIdx.y * NBMAX >= 2) bte2_run_group<T, NBMAX, W, MASKED>(P, CF, bte2_smem_raw, &s_bars, &s_unit);
-  else bte2_run_group<T, 1, W, MASKED>(P, CF, bte2_smem_raw, &s_bars, &s_unit);
 }
 
 // ------------------------------------------------------------------ boundary kernels (v2 layouts)
@@ -836,7 +826,7 @@ __global__ void bte2_ghost_kernel(const __grid_constant__ Bte2Dev P) {
     for (int sl = 0; sl < 4; ++sl) H += (double)hp[sl];
     Gi[e] = (T)(H / P.Pi_face[P.iface_info[fid]]);
   }
-  if (gtid < BTE2_MAXB) P.ticket[gtid] = 0;
+  if (gtid == 0) *P.ticket = 0;
 }
 
 // ------------------------------------------------------------------ (c) update + residual, v2 layouts
@@ -894,9 +884,10 @@ __global__ void bte2_skew_kernel(const __grid_constant__ Bte2Dev P, const double
     for (int cl = 0; cl < 4; ++cl) {
       Bte2Pair<T> *d = reinterpret_cast<Bte2Pair<T> *>(P.dTQ[cl]) +
                        sk2_index(P.nty, P.NU, (cl & 1) ? P.nx - 1 - i : i, (cl & 2) ? P.ny - 1 - j : j, k);
-      if (which == 0) d->y = (T)(src[c % P.src_mod] * scale); else d->x = (T)src[c % P.src_mod];
+      const bool solid = !P.code || (P.code[c] & 1);    // void cells hold 0 (bte.h: "void cells 0")
+      if (which == 0) d->y = (T)(src[c % P.src_mod] * scale); else d->x = solid ? (T)src[c % P.src_mod] : (T)0;
     }
-    if (which == 1) P.dT[c] = src[c % P.src_mod];
+    if (which == 1) P.dT[c] = (!P.code || (P.code[c] & 1)) ? src[c % P.src_mod] : 0.0;
   }
 }
 #endif  // __CUDACC__

@@ -76,7 +76,7 @@ def check(bte, p, n, precision=None, checkpoints=(), res_rtol=None):
         assert eT <= tol, f"{p.name} n={stop}: err_T={eT:.3e} > {tol}"
         assert eq <= tol, f"{p.name} n={stop}: err_q={eq:.3e} > {tol}"
         # Eq. 23 residuals: same definition on both sides
-        rt = res_rtol if res_rtol is not None else (1e-6 if prec == W.FP64 else 2e-2)
+        rt = res_rtol if res_rtol is not None else (1e-6 if prec == W.FP64 else 1e-4)
         if rT > 1e3 * tol and np.isfinite(rT):
             assert abs(gT - rT) <= rt * rT, f"{p.name} n={stop}: eps_T {gT} vs {rT}"
         if rq > 1e3 * tol and np.isfinite(rq):
@@ -262,21 +262,24 @@ def test_config0_full_matches_oracle_and_golden(bte):
 
 @pytest.mark.slow
 def test_config1_full(bte):
+    """Full-size config 1 at n = 50 (parity at n = 50)."""
     p = W.config(1)
-    check(bte, p, 20, checkpoints=(1,))
+    check(bte, p, 50, checkpoints=(1, 10))
 
 
 @pytest.mark.slow
 @pytest.mark.parametrize("prec", [W.FP64, W.FP32_STORE_FP64_ACC])
 def test_config2_full(bte, prec):
+    """Full-size config 2 at n = 50 in both precisions."""
     p = W.config(2)
-    check(bte, p, 6, precision=prec, checkpoints=(1,))
+    check(bte, p, 50, precision=prec, checkpoints=(1, 10))
 
 
 @pytest.mark.slow
 def test_config3_full(bte):
+    """Full-size config 3 (voxel mask, diffuse interfaces, periodic x) at n = 50."""
     p = W.config(3)
-    check(bte, p, 5, checkpoints=(1,))
+    check(bte, p, 50, checkpoints=(1, 10))
 
 
 @pytest.mark.slow
@@ -292,11 +295,24 @@ def test_config4_full_sampled(bte):
 @pytest.mark.slow
 @pytest.mark.parametrize("prec", [W.FP64, W.FP32_STORE_FP64_ACC])
 def test_config4_replica_converged_state(bte, prec):
-    """Like-for-like converged-state check: a 32x16x16 replica of the large slab is
-    iterated far towards its fixed point on both sides; rounding differences must not accumulate."""
-    p = W.config(4, grid=(32, 16, 16))
-    out = check(bte, p, 400, precision=prec, checkpoints=(100,))
-    assert out[-1][3][0] < 1e-5          # oracle eps_T: well converged
+    """Like-for-like converged-state check: the 64x32x32 replica of the large slab is run to
+    eps_T <= 1e-8 on BOTH sides (same iteration count, checked every 50 iterations); rounding differences must not
+    accumulate over the ~10^3 iterations, in either precision."""
+    import oracle
+    p = W.config(4, grid=(64, 32, 32))
+    ref = oracle.RefSolver(p, threads=NCPU)
+    gpu = bte.Solver(p, precision=prec)
+    n = 0
+    while n < 4000:
+        ref.iterate(50); gpu.iterate(50); n += 50
+        if ref.residual()[0] <= 1e-8:
+            break
+    rT, _ = ref.residual()
+    gT, _ = gpu.residual()
+    assert rT <= 1e-8, f"oracle did not converge in {n} iterations (eps_T = {rT})"
+    assert gT <= (1.05e-8 if prec == W.FP64 else 1e-6)      # fp32: the residual floors at the fp32 rounding level
+    eT, eq = errors(gpu.temperature().cpu().numpy(), gpu.heat_flux().cpu().numpy(), ref.temperature(), ref.heat_flux())
+    assert eT <= TOL[prec] and eq <= TOL[prec], (n, eT, eq)
 
 
 @pytest.mark.slow
@@ -368,3 +384,100 @@ def test_config4_full_converged_energy_balance(bte):
     fine, tmin = balance(None)
     assert abs(1 - fine) < 0.03 and abs(1 - fine) < abs(1 - coarse) < 0.09
     assert tmin >= 0.0                                               # heating only: no undershoot below the wall
+
+
+# ---------------------------------------------------------------- generic path beyond one chunk / 16 bands
+def test_generic_path_two_direction_chunks_per_octant(bte):
+    """32 directions per octant (8 polar x 32 azimuth: two chunks of 16 on the generic path, hemispherical partial sums
+    from 2 x 4 slots) on a masked grid with diffuse interfaces and a diffuse box face."""
+    p = W.random_problem(11, dim=3, shape=(13, 11, 9), masked=True, interface_type=W.BC_DIFFUSE,
+                         bc_types=(W.BC_ISOTHERMAL, W.BC_DIFFUSE), n_polar=8, n_azimuth=32)
+    assert len(p.w) == 256
+    g = bte.Solver(p)
+    assert g.kernel_path == 1
+    check(bte, p, 12, precision=W.FP64, checkpoints=(1, 3))
+    check(bte, p, 12, precision=W.FP32_STORE_FP64_ACC)
+
+
+def test_generic_path_seventeen_bands(bte):
+    """More than 16 bands (the fast path's parameter table holds 16): generic path, masked grid, diffuse interface."""
+    p = W.random_problem(12, dim=3, shape=(12, 10, 8), n_bands=17, masked=True, interface_type=W.BC_DIFFUSE,
+                         n_polar=8, n_azimuth=16)
+    assert len(p.C) == 17
+    g = bte.Solver(p)
+    assert g.kernel_path == 1
+    check(bte, p, 12, precision=W.FP64, checkpoints=(1, 3))
+    check(bte, p, 12, precision=W.FP32_STORE_FP64_ACC)
+
+
+# ---------------------------------------------------------------- reading G15 where it is weakest
+def test_fp32_moments_antisymmetric_fifteen_bands(bte):
+    """G15 as built: on the fast path the moments of ONE octant are summed in fp32 over 16 directions and all bands
+    (tau spans three decades, so the 1/tau weights of M0 span three decades too).  Attacked where it is weakest: an
+    antisymmetric +-dT_w film problem (signed intensities that cancel in M0, dT crosses zero) with the 15-band table,
+    far into the iteration; error norm G12 against the fp64 oracle, and against the fp64 GPU path."""
+    p = W.config(4, grid=(48, 34, 20))
+    p.Q = None
+    p.face_bc = [(W.BC_ISOTHERMAL, 0.5), (W.BC_ISOTHERMAL, -0.5), (W.BC_SPECULAR, 0.0), (W.BC_SPECULAR, 0.0),
+                 (W.BC_SPECULAR, 0.0), (W.BC_SPECULAR, 0.0)]
+    assert bte.Solver(p).kernel_path == 2
+    out = check(bte, p, 300, precision=W.FP32_STORE_FP64_ACC, checkpoints=(5, 50))
+    assert out[-1][1] <= 2e-5 and out[-1][2] <= 2e-5          # measured ~1e-6: an order of magnitude of margin
+    a = bte.Solver(p, precision=W.FP64); a.iterate(300)
+    b = bte.Solver(p, precision=W.FP32_STORE_FP64_ACC); b.iterate(300)
+    eT, eq = errors(b.temperature().cpu().numpy(), b.heat_flux().cpu().numpy(),
+                    a.temperature().cpu().numpy(), a.heat_flux().cpu().numpy())
+    assert eT <= 2e-5 and eq <= 2e-5
+    # antisymmetry about the mid-plane survives in fp32 to the same level
+    dT = b.temperature().cpu().numpy()
+    assert np.abs(dT + dT[:, :, ::-1]).max() <= 2e-5 * np.abs(dT).max()
+
+
+@pytest.mark.slow
+def test_config4_full_fp32_vs_fp64_gpu(bte):
+    """Full-size config 4: the fp32-storage path against the fp64 GPU path (itself checked against the oracle at n = 5)
+    at n = 5 and far into the iteration (n = 200), reading G15, tolerance 1e-4."""
+    p = W.config(4)
+    a = bte.Solver(p, precision=W.FP64)
+    b = bte.Solver(p, precision=W.FP32_STORE_FP64_ACC)
+    for n in (5, 195):
+        a.iterate(n); b.iterate(n)
+        eT, eq = errors(b.temperature().cpu().numpy(), b.heat_flux().cpu().numpy(),
+                        a.temperature().cpu().numpy(), a.heat_flux().cpu().numpy())
+        assert eT <= 1e-4 and eq <= 1e-4, (a.iterations_done, eT, eq)
+
+
+def test_set_temperature_masks_void_cells(bte):
+    """bte_set_temperature with nonzero values on void cells: void cells read 0 on both kernel paths (bte.h)."""
+    import oracle
+    for grid in ((12, 10, 8), (11, 9, 7)):              # fast (masked) / generic
+        p = W.config(3, grid=grid)
+        rng = np.random.default_rng(3)
+        dT0 = rng.uniform(0.5, 1.0, size=(p.nz, p.ny, p.nx))          # nonzero everywhere, void cells included
+        g = bte.Solver(p, precision=W.FP64)
+        g.set_temperature(dT0)
+        t = g.temperature().cpu().numpy()
+        assert not t[p.mask == 0].any() and (t[p.mask == 1] == dT0[p.mask == 1]).all()
+        ref = oracle.RefSolver(p); ref.set_temperature(dT0 * p.mask); ref.iterate(2)
+        g.iterate(2)
+        eT, eq = errors(g.temperature().cpu().numpy(), g.heat_flux().cpu().numpy(), ref.temperature(), ref.heat_flux())
+        assert eT <= 1e-10 and eq <= 1e-10
+
+
+def test_g14_directions_in_a_coordinate_plane(bte):
+    """Reading G14 on the CUDA path: a quadrature with directions that have s_x = 0 or s_y = 0 exactly (azimuth offset
+    0; isothermal faces only, such a table is not reflection-closed per octant), against the oracle."""
+    mu, wmu = np.polynomial.legendre.leggauss(4)
+    s, w = [], []
+    for m, wm in zip(mu, wmu):
+        st = np.sqrt(1.0 - m * m)
+        for k in range(8):
+            cx, cy = np.cos(k * np.pi / 4), np.sin(k * np.pi / 4)
+            cx = 0.0 if abs(cx) < 1e-12 else cx
+            cy = 0.0 if abs(cy) < 1e-12 else cy
+            s.append((st * cx, st * cy, m)); w.append(wm * np.pi / 4)
+    p = W.config(2, grid=(9, 8, 7))
+    p.s, p.w = np.array(s), np.array(w)
+    p.face_bc = [(W.BC_ISOTHERMAL, 0.1 * f) for f in range(6)]
+    check(bte, p, 10, precision=W.FP64, checkpoints=(1, 2))
+    check(bte, p, 10, precision=W.FP32_STORE_FP64_ACC)

@@ -32,7 +32,7 @@ def test_ticket_order_is_topological_for_any_cta_count(slots, prec):
         assert info["band_groups"] == groups
         tiles = -(-p.ny // 64) * -(-p.nz // (2 * info["warps_per_cta"]))
         assert info["work_units"] == 8 * groups * tiles
-        assert info["steps_per_unit"] == p.nx + 32 + info["warps_per_cta"] - 1   # nx + 32 local steps per warp, warps one step apart
+        assert info["steps_per_unit"] == p.nx + 31 + info["warps_per_cta"] - 1
 
 
 def test_fast_path_needs_symmetric_16_direction_octants_and_few_bands():
