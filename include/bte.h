@@ -45,8 +45,9 @@ typedef enum {
                               reflection that does not map the direction set onto itself (equal weights) */
   BTE_ERR_WORKSPACE = 3,   /* workspace NULL, misaligned (256 B) or smaller than bte_workspace_bytes */
   BTE_ERR_CUDA = 4,        /* any CUDA runtime error (bte_last_cuda_error gives the code) */
-  BTE_ERR_UNSUPPORTED = 5  /* valid problem outside this build: SPECULAR interface_bc; coefficient table
+  BTE_ERR_UNSUPPORTED = 5, /* valid problem outside this build: SPECULAR interface_bc; coefficient table
                               larger than the constant bank (non-mirror-symmetric quadrature x many bands) */
+  BTE_ERR_TOO_LARGE = 6    /* bte_residual_static only: n_cells > BTE_STATIC_MAX_CELLS */
 } bte_status;
 
 /* Eq. 5 / Eq. 6 / Eq. 7; PERIODIC: BASELINE.json configs[3] */
@@ -151,6 +152,24 @@ int32_t bte_last_cuda_error(void);
 typedef enum { BTE_OPT_FORCE_GENERIC = 0, BTE_OPT_WARPS = 1, BTE_OPT_PUBLISH_PERIOD = 2, BTE_OPT_START_SLACK = 3,
                BTE_OPT_SCHEDULE = 4, BTE_OPT_COUNT_ = 5 } bte_option;
 bte_status bte_set_option(int32_t option, int32_t value);
+
+/* Allocation-free stopping test, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it) and so cannot hold a bte_solver workspace: eps_T, eps_q of Eq. 23 (
+ * N = solid cells, maxima over solid cells of the NEW snapshot, |q| magnitudes; 0/0 -> 0, x/0 -> +inf) between two
+ * snapshots the caller holds -- the numbers bte_residual reports when the snapshots are bte_get_temperature /
+ * bte_get_heat_flux taken before and after one bte_iterate(h, 1, .).
+ *   d_dT_new, d_dT_old: device, [n_cells];  d_q_new, d_q_old: device, [3][n_cells];
+ *   d_solid_mask: device, [n_cells], 1 = solid, or NULL = all solid;  d_eps: device, [2] = {eps_T, eps_q}.
+ * One memset node + one kernel, asynchronous on cuda_stream; calls no cudaMalloc / cudaFree and no allocating library
+ * routine.  The per-block partial sums live in a file-scope __device__ array of the library (164 096 B, held by every
+ * GPU that loads the library until the process exits; its address is resolved once per device by the first call made
+ * with that device current).  LIMIT: n_cells <= BTE_STATIC_MAX_CELLS, else BTE_ERR_TOO_LARGE and nothing is launched.
+ * All calls on one device share that array: calls that may overlap on the GPU (different streams or threads) race --
+ * serialise them.  The result does not depend on what an earlier call left in the array. */
+#define BTE_STATIC_MAX_CELLS (1 << 24) /* 16 777 216 cells (configs[4] has 256*128*128 = 4 194 304) */
+bte_status bte_residual_static(const double *d_dT_new, const double *d_dT_old, const double *d_q_new,
+                               const double *d_q_old, const uint8_t *d_solid_mask, int64_t n_cells, double *d_eps,
+                               void *cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -19,21 +19,21 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _SO = os.path.join(_HERE, "libbte_b200.so")
-_SOURCES = [os.path.join(_CSRC, f) for f in ("bte_api.cu", "bte_kernels.cuh", "bte_sweep2.cuh", "bte_internal.h")] + \
+_SOURCES = [os.path.join(_CSRC, f) for f in ("bte_api.cu", "bte_kernels.cuh", "bte_sweep2.cuh", "bte_static.cuh", "bte_internal.h")] + \
            [os.path.join(os.path.dirname(_HERE), "include", "bte.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]
 
 STATUS = {0: "BTE_OK", 1: "BTE_ERR_INVALID_ARG", 2: "BTE_ERR_QUADRATURE", 3: "BTE_ERR_WORKSPACE",
-          4: "BTE_ERR_CUDA", 5: "BTE_ERR_UNSUPPORTED"}
+          4: "BTE_ERR_CUDA", 5: "BTE_ERR_UNSUPPORTED", 6: "BTE_ERR_TOO_LARGE"}
 BTE_FP64, BTE_FP32_STORE_FP64_ACC = 0, 1
 
 EXPORTS = ["bte_workspace_bytes", "bte_create", "bte_iterate", "bte_get_temperature", "bte_get_heat_flux",
            "bte_set_temperature", "bte_residual", "bte_solve_host", "bte_set_sweep_timing",
            "bte_get_sweep_timing", "bte_updates_per_sweep",
            "bte_iterations_done", "bte_kernel_launches_per_iteration", "bte_kernel_path", "bte_plan_info", "bte_schedule_info", "bte_destroy",
-           "bte_status_string", "bte_last_cuda_error", "bte_set_option"]
+           "bte_status_string", "bte_last_cuda_error", "bte_set_option", "bte_residual_static"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -110,6 +110,7 @@ def lib():
         L.bte_status_string.restype = C.c_char_p
         L.bte_last_cuda_error.restype = i32
         L.bte_set_option.argtypes = [i32, i32]
+        L.bte_residual_static.argtypes = [vp, vp, vp, vp, vp, i64, vp, vp]
         _lib = L
     return _lib
 
@@ -122,6 +123,31 @@ def bte_set_option(name, value) -> None:
     rc = lib().bte_set_option(OPTIONS[name], int(value))
     if rc:
         raise BteError(rc, "bte_set_option")
+
+
+STATIC_MAX_CELLS = 1 << 24
+
+
+def bte_residual_static(dT_new, dT_old, q_new, q_old, solid_mask, eps_out, stream=None) -> None:
+    """Allocation-free Eq. 23 stopping test (include/bte.h bte_residual_static).  Every argument is a contiguous CUDA
+    tensor the caller owns: dT_* float64 [n_cells], q_* float64 [3][n_cells], solid_mask uint8 [n_cells] or None,
+    eps_out float64 [2] (receives eps_T, eps_q).  Asynchronous on `stream` (default: torch's current stream)."""
+    import torch
+    for t, dt in ((dT_new, torch.float64), (dT_old, torch.float64), (q_new, torch.float64), (q_old, torch.float64),
+                  (eps_out, torch.float64)) + (() if solid_mask is None else ((solid_mask, torch.uint8),)):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == dt):
+            raise ValueError("bte_residual_static takes contiguous CUDA tensors (float64; uint8 mask)")
+    n = dT_new.numel()
+    if dT_old.numel() != n or q_new.numel() != 3 * n or q_old.numel() != 3 * n or eps_out.numel() < 2 or \
+            (solid_mask is not None and solid_mask.numel() != n):
+        raise ValueError("bte_residual_static: sizes do not match")
+    s = torch.cuda.current_stream(dT_new.device) if stream is None else stream
+    with torch.cuda.device(dT_new.device):
+        rc = lib().bte_residual_static(dT_new.data_ptr(), dT_old.data_ptr(), q_new.data_ptr(), q_old.data_ptr(),
+                                       None if solid_mask is None else solid_mask.data_ptr(), n, eps_out.data_ptr(),
+                                       C.c_void_p(s.cuda_stream))
+    if rc:
+        raise BteError(rc, "bte_residual_static")
 
 
 def _marshal(p, precision=None):

@@ -974,6 +974,7 @@ const char *bte_status_string(bte_status s) {
     case BTE_ERR_WORKSPACE: return "workspace too small or misaligned";
     case BTE_ERR_CUDA: return "CUDA error";
     case BTE_ERR_UNSUPPORTED: return "unsupported problem";
+    case BTE_ERR_TOO_LARGE: return "size beyond the static scratch array (n_cells > BTE_STATIC_MAX_CELLS)";
   }
   return "unknown";
 }
@@ -986,3 +987,6 @@ bte_status bte_set_option(int32_t option, int32_t value) {
 }
 
 }  // extern "C"
+
+// the allocation-free entry point (bte_residual_static) and its file-scope __device__ scratch array
+#include "bte_static.cuh"
