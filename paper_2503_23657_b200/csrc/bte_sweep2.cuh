@@ -148,6 +148,11 @@ __device__ __forceinline__ int ld_acquire_gpu(const int *p) {
   asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
+__device__ __forceinline__ int ld_relaxed_gpu(const int *p) {
+  int v;
+  asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
 __device__ __forceinline__ void st_release_gpu(int *p, int v) {
   asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
@@ -272,13 +277,18 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
   Ch *ydst = (ty == P.nty - 1 ? reinterpret_cast<Ch *>(O.ydstN) : reinterpret_cast<Ch *>(O.ypl) + ypl2_index<T>(P, ty + 1, 0, 0, 0, 0, 0, 0)) +
              ypl2_index<T>(P, 0, tz, b0 + (J < 2 * NC ? yb : 0), K, 0, ykk, ych);
 
-  // ---- progress of the units this one follows: lanes 0..2 of warp 0 keep the last value seen in a register
-  const int mydep = tid == 0 ? un.dep_y : (tid == 1 ? un.dep_z : (tid == 2 ? un.dep_prev : -1));
-  const int mylag = tid == 0 ? 33 : (tid == 1 ? W + 1 : 1);
+  // ---- progress of the units this one follows: three poller threads keep the last value seen in a register
+  // the three pollers and the publisher sit in different warps: their memory round trips overlap instead of adding up
+  // in warp 0 (every other warp waits for the slowest one at the step barrier)
+  constexpr int ROLE1 = (1 % W) * 32 + 1 / W, ROLE2 = (2 % W) * 32 + 2 / W, ROLEP = (3 % W) * 32 + 3 / W;
+  const int mydep = tid == 0 ? un.dep_y : (tid == ROLE1 ? un.dep_z : (tid == ROLE2 ? un.dep_prev : -1));
+  const int mylag = tid == 0 ? 33 : (tid == ROLE1 ? W + 1 : 1);
   int seen = 0, peek = 0;
   auto ensure = [&](int t1) {          // everything step t1 reads from other units has been published
     if (mydep >= 0 && !BTE2_DBGBIT(P, 4)) {
-      seen = max(seen, peek - ebase);
+      // the peek is a relaxed load (asynchronous: no L1 invalidation behind it); a publication it shows is then
+      // acquired properly, once per publication instead of once per step
+      if (peek - ebase > seen) seen = max(seen, ld_acquire_gpu(P.prog + mydep) - ebase);
       if (seen < t1 + mylag) {
         int v;
         while ((v = ld_acquire_gpu(P.prog + mydep) - ebase) < t1 + mylag) __nanosleep(64);
@@ -490,7 +500,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     prefetch(t + D, rbp);
     cp_async_commit();
     if (t > 0) copy_out(t - 1);
-    if (tid < 3 && mydep >= 0 && seen < t + 1 + D + mylag) peek = ld_acquire_gpu(P.prog + mydep);   // consumed by ensure() below
+    if (mydep >= 0 && seen < t + 1 + D + mylag) peek = ld_relaxed_gpu(P.prog + mydep);   // consumed by ensure() below
 
     V2 m[2][2][4];                                     // moment partial sums of even / odd directions
 #pragma unroll
@@ -600,7 +610,7 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     if (BTE2_MDIST(T) == 0) cp_async_wait<D - 1>();   // the accumulator content fetched in THIS step has landed
 #if BTE2_SPLITBAR
     cp_async_wait<D - 1>();            // everything step t+1 reads has landed
-    if (tid < 3) ensure(t + 1 + D);    // ... and what step t+1 prefetches has been published upstream
+    if (mydep >= 0) ensure(t + 1 + D);    // ... and what step t+1 prefetches has been published upstream
     mbar_arrive(stepbar);              // this thread's shared-memory reads and writes of step t are done
 #endif
     if (act) {
@@ -651,10 +661,10 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
     __syncwarp();                      // yst rows written after the arrive are read by this warp's copy_out next step
 #else
     cp_async_wait<D - 1>();            // everything step t+1 reads has landed
-    if (tid < 3) ensure(t + 1 + D);    // ... and what step t+1 prefetches has been published upstream
+    if (mydep >= 0) ensure(t + 1 + D);    // ... and what step t+1 prefetches has been published upstream
     __syncthreads();
 #endif
-    if ((t & P.pub_mask) == P.pub_mask && tid == 0) {   // faces and moments of steps < t are in global memory
+    if ((t & P.pub_mask) == P.pub_mask && tid == ROLEP) {   // faces and moments of steps < t are in global memory
       __threadfence();
       st_release_gpu(P.prog + unit, ebase + t);
     }
