@@ -148,11 +148,9 @@ int32_t bte_last_cuda_error(void);
  *   BTE_OPT_START_SLACK     1..256: extra steps a unit lets the units it follows get ahead before it starts
  *   BTE_OPT_SCHEDULE        1: ticket order = band groups of one (tile, octant) consecutively instead of the simulated
  *                           list schedule (experiment on L2 reuse; same results, different timing)
- *   BTE_OPT_SWEEP_KERNEL    1: fast path on the single-role kernel (every warp computes, prefetches and polls) instead of
- *                           the warp-specialised one (compute warps + helper warps; used for 4 or 8 warps per CTA)
  * Returns BTE_ERR_INVALID_ARG for an unknown option. */
 typedef enum { BTE_OPT_FORCE_GENERIC = 0, BTE_OPT_WARPS = 1, BTE_OPT_PUBLISH_PERIOD = 2, BTE_OPT_START_SLACK = 3,
-               BTE_OPT_SCHEDULE = 4, BTE_OPT_SWEEP_KERNEL = 5, BTE_OPT_COUNT_ = 6 } bte_option;
+               BTE_OPT_SCHEDULE = 4, BTE_OPT_COUNT_ = 5 } bte_option;
 bte_status bte_set_option(int32_t option, int32_t value);
 
 /* Allocation-free stopping test, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving

@@ -19,7 +19,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _SO = os.path.join(_HERE, "libbte_b200.so")
-_SOURCES = [os.path.join(_CSRC, f) for f in ("bte_api.cu", "bte_kernels.cuh", "bte_sweep2.cuh", "bte_sweep3.cuh", "bte_static.cuh", "bte_internal.h")] + \
+_SOURCES = [os.path.join(_CSRC, f) for f in ("bte_api.cu", "bte_kernels.cuh", "bte_sweep2.cuh", "bte_static.cuh", "bte_internal.h")] + \
            [os.path.join(os.path.dirname(_HERE), "include", "bte.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -115,7 +115,7 @@ def lib():
     return _lib
 
 
-OPTIONS = {"force_generic": 0, "warps": 1, "publish_period": 2, "start_slack": 3, "schedule": 4, "sweep_kernel": 5}
+OPTIONS = {"force_generic": 0, "warps": 1, "publish_period": 2, "start_slack": 3, "schedule": 4}
 
 
 def bte_set_option(name, value) -> None:

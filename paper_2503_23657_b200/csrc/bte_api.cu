@@ -49,7 +49,6 @@ struct Plan {
   size_t gf_elems = 0;
   // fast path (bte_sweep2.cuh)
   bool v2 = false, masked2 = false;
-  bool ws = false;                       // fast path served by the warp-specialised kernel (bte_sweep3.cuh)
   int layers = 1;                        // 2: a 2-D problem run as a two-layer 3-D slab on the fast path
   int64_t user_ncell = 0, user_nsolid = 0;
   std::vector<uint32_t> codeP[4];
@@ -317,7 +316,6 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
     Bte2Dev &d = pl.d2;
     int W = p->nz >= 48 ? 8 : (p->nz <= 4 ? 2 : 4);   // 2 warps: thin slabs (the two-layer form of 2-D problems)
     { const int w = g_opt[BTE_OPT_WARPS].load(); if (w == 2 || w == 4 || w == 8) W = w; }
-    pl.ws = W >= 4 && g_opt[BTE_OPT_SWEEP_KERNEL].load() != 1;
     d.nx = p->nx; d.ny = p->ny; d.nz = p->nz; d.B = B; d.W = W;
     d.nty = (p->ny + 63) / 64; d.ntz = (p->nz + 2 * W - 1) / (2 * W); d.NU = p->nx + 31;
     d.nsteps = p->nx + 31 + W - 1;
@@ -449,7 +447,7 @@ size_t bind(Plan &pl, unsigned char *ws) {
     pl.state_begin = off;
     d.Gi = d.n_iface ? take((size_t)d.n_iface * d.B * tsz) : nullptr;
     d.Hd = (d.n_iface && d.iface_type == 1) ? take((size_t)6 * N * d.B * 4 * tsz) : nullptr;
-    d.prog = (int32_t *)take((size_t)d.n_units * d.W * 4);   // per warp (bte_sweep3.cuh); the single-role kernel uses [unit]
+    d.prog = (int32_t *)take((size_t)d.n_units * 4);
     d.ticket = (int32_t *)take(256);
     dv.red = (double *)take((size_t)(4 * dv.n_red_blocks + 4) * 8);
     dv.dT = (double *)take(N * 8);
@@ -512,8 +510,7 @@ void order_units2(Plan &pl, int slots) {
   }
   auto allowed = [&](int u) {
     const int deps[3] = {U[u].dep_y, U[u].dep_z, U[u].dep_prev};
-    const int el = pl.ws ? BTE3_ELAG : 0;
-    const int lag[3] = {33 + el, W + 1 + el, 1 + el};
+    const int lag[3] = {33, W + 1, 1};
     double a = 0;
     for (int k = 0; k < 3; ++k)
       if (deps[k] >= 0) a = std::max(a, start[deps[k]] + (lag[k] + (pl.dev.fp32 ? BTE2_DIST(W, float) : BTE2_DIST(W, double)) + pl.d2.slack + pl.d2.pub_mask + 1) * steptime[deps[k]]);
@@ -607,13 +604,7 @@ bte_status skew(bte_solver *h, const double *src, double scale, int which, cudaS
 }
 
 template <typename T, int W>
-void launch_sweep3(bte_solver *h, const Bte2Coefs<T> &cf, cudaStream_t st) {
-  if (h->pl.masked2) bte3_sweep_kernel<T, W, true><<<h->sweep_grid, BTE3_THREADS(W), h->pl.smem2, st>>>(h->pl.d2, cf);
-  else bte3_sweep_kernel<T, W, false><<<h->sweep_grid, BTE3_THREADS(W), h->pl.smem2, st>>>(h->pl.d2, cf);
-}
-template <typename T, int W>
 void launch_sweep2(bte_solver *h, const Bte2Coefs<T> &cf, cudaStream_t st) {
-  if (W >= 4 && h->pl.ws) { launch_sweep3<T, (W >= 4 ? W : 4)>(h, cf, st); return; }
   if (h->pl.masked2) bte2_sweep_kernel<T, W, true><<<h->sweep_grid, W * 32, h->pl.smem2, st>>>(h->pl.d2, cf);
   else bte2_sweep_kernel<T, W, false><<<h->sweep_grid, W * 32, h->pl.smem2, st>>>(h->pl.d2, cf);
 }
@@ -625,7 +616,7 @@ bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t
   const int bgrid = h->num_sms * 8;
   for (int it = 0; it < n; ++it) {
     const int ep = (int)(h->iters % 30000) + 1;
-    if (ep == 1 && h->iters > 0) CK(cudaMemsetAsync(d.prog, 0, (size_t)d.n_units * d.W * 4, st));
+    if (ep == 1 && h->iters > 0) CK(cudaMemsetAsync(d.prog, 0, (size_t)d.n_units * 4, st));
     d.epoch = ep;
     d.fill_iso = h->iters == 0;
     {   // ghost planes to fill: diffuse faces every iteration, isothermal faces once (specular / periodic: none)
@@ -677,26 +668,8 @@ bte_status iterate2_T(bte_solver *h, int n, const Bte2Coefs<T> &cf, cudaStream_t
 }
 
 template <typename T, int W>
-bte_status setup_sweep3_W(bte_solver *h) {
-  Plan &pl = h->pl;
-  pl.smem2 = sizeof(Bte3Smem<T, sizeof(T) == 4 ? 2 : 1, W, BTE3_RING(T)>);
-  int occ = 0;
-  if (pl.masked2) {
-    CK(cudaFuncSetAttribute(bte3_sweep_kernel<T, W, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem2));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bte3_sweep_kernel<T, W, true>, BTE3_THREADS(W), pl.smem2));
-  } else {
-    CK(cudaFuncSetAttribute(bte3_sweep_kernel<T, W, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem2));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bte3_sweep_kernel<T, W, false>, BTE3_THREADS(W), pl.smem2));
-  }
-  if (occ < 1) { g_last_cuda.store((int)cudaErrorLaunchOutOfResources); return BTE_ERR_CUDA; }
-  h->sweep_grid = (int)std::min<int64_t>(pl.d2.n_units, (int64_t)h->num_sms * occ);
-  pl.nthreads = BTE3_THREADS(W);
-  return BTE_OK;
-}
-template <typename T, int W>
 bte_status setup_sweep2_W(bte_solver *h) {
   Plan &pl = h->pl;
-  if (W >= 4 && pl.ws) return setup_sweep3_W<T, (W >= 4 ? W : 4)>(h);
   pl.smem2 = sizeof(Bte2Smem<T, sizeof(T) == 4 ? 2 : 1, W, BTE2_DIST(W, T)>);
   int occ = 0;
   if (pl.masked2) {

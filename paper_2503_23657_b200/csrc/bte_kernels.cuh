@@ -487,4 +487,3 @@ __global__ void bte_skew_kernel(const __grid_constant__ BteDev P, const double *
 }
 
 #include "bte_sweep2.cuh"
-#include "bte_sweep3.cuh"
