@@ -144,7 +144,7 @@ int32_t bte_last_cuda_error(void);
  * already created are not affected).  The library never reads the environment.  value 0 = default.
  *   BTE_OPT_FORCE_GENERIC   1: use the generic kernels for every problem
  *   BTE_OPT_WARPS           2 | 4 | 8: warps per CTA of the fast path (default: by nz)
- *   BTE_OPT_PUBLISH_PERIOD  4 | 8 | 16 | 32: steps between progress publications of a unit (default 8; 4 if nx <= 96)
+ *   BTE_OPT_PUBLISH_PERIOD  4 | 8 | 16 | 32: steps between progress publications of a unit (default: 4 if nx < 224, 8 if nx < 256, else 16)
  *   BTE_OPT_START_SLACK     1..256: extra steps a unit lets the units it follows get ahead before it starts
  *   BTE_OPT_SCHEDULE        1: ticket order = band groups of one (tile, octant) consecutively instead of the simulated
  *                           list schedule (experiment on L2 reuse; same results, different timing)

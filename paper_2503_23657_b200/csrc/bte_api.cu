@@ -299,7 +299,7 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
 
   // ---- fast path: 3-D, all solid, 16 directions in each of the 8 octants with identical |s|, w tables
   // (mirror-symmetric quadrature), <= 16 bands.  Anything else runs the generic kernels above.
-  bool v2 = p->dim == 3 && B <= BTE2_MAXB && p->nx <= 60000 && p->ny % 2 == 0 && p->nz % 2 == 0;
+  bool v2 = p->dim == 3 && B <= BTE2_MAXB && p->nx <= 60000 && p->ny % 2 == 0 && p->nz % 2 == 0 && N < (int64_t)1 << 31;   // (32-bit cell index in the update kernel)
   pl.masked2 = nsolid != N;
   if (g_opt[BTE_OPT_FORCE_GENERIC].load() == 1) v2 = false;
   for (int o = 0; o < 8 && v2; ++o) {
@@ -319,7 +319,9 @@ bte_status build_plan_impl(const bte_problem *p, Plan &pl) {
     d.nx = p->nx; d.ny = p->ny; d.nz = p->nz; d.B = B; d.W = W;
     d.nty = (p->ny + 63) / 64; d.ntz = (p->nz + 2 * W - 1) / (2 * W); d.NU = p->nx + 31;
     d.nsteps = p->nx + 31 + W - 1;
-    d.pub_mask = (p->nx <= 96 ? BTE2_PUB / 2 : BTE2_PUB) - 1; d.slack = BTE2_SLACK;   // short rows: publish progress twice as often (measured)
+    // publication period of a unit's progress (measured, profiles/README.md): short and medium rows gain from frequent
+    // publication (the units behind start and follow more closely: configs 1-3 -6 ... -8 %), long rows from fewer fences
+    d.pub_mask = (p->nx < 224 ? BTE2_PUB / 2 : (p->nx < 256 ? BTE2_PUB : 2 * BTE2_PUB)) - 1; d.slack = BTE2_SLACK;
     { const int v = g_opt[BTE_OPT_PUBLISH_PERIOD].load(); if (v == 4 || v == 8 || v == 16 || v == 32) d.pub_mask = v - 1; }
     { const int v = g_opt[BTE_OPT_START_SLACK].load(); if (v > 0 && v <= 256) d.slack = v; }
     d.NS = (int64_t)p->nz * d.nty * d.NU * 64;

@@ -845,9 +845,12 @@ __global__ void bte2_ghost_kernel(const __grid_constant__ Bte2Dev P) {
 template <typename T>
 __global__ void __launch_bounds__(256, 4) bte2_update_kernel(const __grid_constant__ Bte2Dev P) {
   double sT = 0, mT = 0, sq = 0, mq = 0;
-  for (int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; c < P.ncell; c += (int64_t)gridDim.x * blockDim.x) {
+  // 32-bit cell index (host check: ncell < 2^31): the 64-bit divisions of the first version kept the XU pipe half busy
+  const unsigned ncell = (unsigned)P.ncell, nxu = (unsigned)P.nx, nyu = (unsigned)P.ny;
+  for (unsigned c = blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += gridDim.x * blockDim.x) {
     if (P.code && !(P.code[c] & 1)) continue;          // void cell: dT, q stay 0
-    const int i = (int)(c % P.nx), j = (int)((c / P.nx) % P.ny), k = (int)(c / ((int64_t)P.nx * P.ny));
+    const unsigned row = c / nxu;
+    const int i = (int)(c - row * nxu), k = (int)(row / nyu), j = (int)(row - (unsigned)k * nyu);
     int64_t sk[4];
 #pragma unroll
     for (int cl = 0; cl < 4; ++cl)
