@@ -598,7 +598,8 @@ __device__ __forceinline__ void bte2_run_unit(const Bte2Dev &P, const Bte2Coefs<
             }
           }
         }
-      } else if (fast) {
+      } else if (fast && !MASKED) {   // (the masked kernel does without this copy of the arithmetic: at ~10,000 instructions
+                                      // it is bound by instruction fetch, and dropping it took config 3 from 2.47 to 2.24 ms)
 #pragma unroll
         for (int ch = 0; ch < NCH; ++ch) chunk(std::true_type{}, b, ch, r, m, rb, cur, true, zrd, zwr);
       } else {
